@@ -1,0 +1,118 @@
+/* vc.h — C ABI of libvc.so: the GKR/CMT prover hot path over F_p, p = 2^61 - 1, on one B200.
+ *
+ * Protocol: PAPER.md:93-101 (§3.1, GKR iteration structure), PAPER.md:121-123 (§4.1.1, each gate
+ * contributes independently to each message; contributions are reduced in F_p), PAPER.md:197 (§6.1,
+ * the field).  Conventions the paper leaves open follow SURVEY.md §8(c) / DESIGN.md "Readings".
+ *
+ * Conventions: layer 0 = outputs, layer d = inputs; layer i has exactly 2^log_size gates; gate g of
+ * layer i reads entries in1[g], in2[g] of layer i+1.  All field words are canonical uint64 in [0,p).
+ * Bit k of an index is variable k (k = 0 least significant).  Challenges are H(seed, ctr++) from a
+ * counter-based generator kept on the device (splitmix64 stream, low 61 bits, p -> 0).
+ *
+ * Every function returns an integer code (VC_OK = 0); nothing throws, aborts or prints.
+ * Functions taking a `cuda_stream` (a cudaStream_t passed as void*, NULL = default stream) only
+ * ENQUEUE work and return without synchronising; VC_OK then means "enqueued".
+ * There is no CPU fallback: without a CUDA device every compute entry point returns VC_ERR_CUDA.
+ */
+#ifndef VC_H
+#define VC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vc_circuit vc_circuit; /* opaque; owns device copies of records, V tables, scratch, proof state */
+
+enum { VC_OK = 0, VC_ERR_ARG = 1, VC_ERR_SHAPE = 2, VC_ERR_STATE = 3, VC_ERR_CUDA = 4, VC_ERR_NOMEM = 5 };
+enum { VC_ADD = 0, VC_MULT = 1, VC_SUB = 2, VC_RELAY = 3 };
+
+/* One layer's gate records, structure-of-arrays, in HOST memory (copied at load; caller keeps ownership). */
+typedef struct {
+    uint32_t log_size;    /* the layer has exactly 2^log_size gates */
+    const uint8_t *type;  /* VC_ADD L+R, VC_MULT L*R, VC_SUB L-R, VC_RELAY L */
+    const uint32_t *in1;  /* indices into the layer below, < 2^log_size(below) */
+    const uint32_t *in2;
+} vc_layer;
+
+/* vc_circuit_load — copy the circuit to the device and allocate every buffer the path needs
+ * (value tables V_0..V_d, weights, fold tables, partials, proof state).  Allocation is outside any
+ * timed region (scratch allocation is not counted).  "No-copying approach",
+ * PAPER.md:153 (§5.1.1): the whole circuit stays resident in HBM.
+ *   layers[0] = output layer ... layers[d-1] = the layer fed by the input; log_input = log2(#inputs).
+ * Errors: VC_ERR_ARG (null, d = 0), VC_ERR_SHAPE (log_size > 30, a layer below of size 1, index out
+ * of range, unknown type), VC_ERR_CUDA / VC_ERR_NOMEM. */
+int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit **out);
+
+/* vc_evaluate — layered circuit evaluation (step a1; §6.2.4):
+ * V_d = input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]).
+ *   d_input   DEVICE pointer, 2^log_input canonical words (read; a non-canonical word makes the
+ *             next vc_prove_layer fail with VC_ERR_ARG once the flag is read back — see vc_status).
+ *   d_outputs DEVICE pointer, 2^log_size(layer 0) words (written); may be NULL.
+ * Resets the proof state (next vc_prove_layer must be layer 0). */
+int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, void *cuda_stream);
+
+/* vc_prove_layer — one GKR iteration (steps a2-a7):
+ * layer 0 first resets the challenge counter, draws z_0 and forms the start claim V~_0(z_0);
+ * then beta(z,.) weights, 2*s sum-check rounds (s = log2 size of layer i+1; phase 1 binds the bits of
+ * in1, phase 2 the bits of in2, LSB first; each round emits G[0],G[1],G[2] = the round polynomial at
+ * t = 0,1,2, reduced mod p over all gates, then draws the challenge on the device), then the line
+ * restriction q[0..s] = V~_{i+1}(r1 + t (r2 - r1)), a draw tau, z <- l(tau), claim <- q(tau).
+ *   d_transcript DEVICE pointer, receives 7*s+1 words: 2s x (G0,G1,G2), then q[0..s].
+ *   cap_words    capacity of d_transcript in words (VC_ERR_ARG if < 7*s+1).
+ * Must be called with layer = 0,1,...,d-1 in order after vc_evaluate, with the same seed
+ * (else VC_ERR_STATE).  Leaves (z, claim, counter) on the device for the next call. */
+int vc_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_transcript, uint64_t cap_words,
+                   void *cuda_stream);
+
+/* vc_prove — convenience: vc_prove_layer for layers 0..d-1 into one device buffer (layer 0 first),
+ * cap_words >= vc_total_transcript_words.  Same kernels, same order; no host round-trip. */
+int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, uint64_t cap_words, void *cuda_stream);
+
+/* vc_run_host — the end-to-end call with HOST buffers: H2D copy of the input, vc_evaluate, vc_prove,
+ * D2H copy of outputs and transcript, stream synchronised before returning.
+ *   h_input 2^log_input words (read), h_outputs 2^log_size(layer 0) words (written),
+ *   h_transcript cap_words words (written).  Pinned host memory makes the copies asynchronous. */
+int vc_run_host(vc_circuit *c, const uint64_t *h_input, uint64_t seed, uint64_t *h_outputs,
+                uint64_t *h_transcript, uint64_t cap_words, void *cuda_stream);
+
+/* vc_verify_transcript — the verifier (PAPER.md:63-65 §2.2, :99; host code, not on the hot path).
+ * Recomputes the start claim from h_outputs, checks every round (G0+G1 = claim), the wiring check
+ * after 2s rounds with v1 = q[0], v2 = q[1], follows the line to the next layer, and closes with
+ * claim = V~_d(z) of h_input.  All pointers HOST.  Rejection is NOT an error: returns VC_OK with
+ * *accept = 0 and (fail_layer, fail_round): round m < 2s = round check m failed; round 2s = wiring
+ * check failed; fail_layer = d = closing input check failed. */
+int vc_verify_transcript(const vc_circuit *c, const uint64_t *h_input, const uint64_t *h_outputs, uint64_t seed,
+                         const uint64_t *h_transcript, uint64_t n_words, int *accept, uint32_t *fail_layer,
+                         uint32_t *fail_round);
+
+void vc_circuit_free(vc_circuit *c);
+const char *vc_strerror(int code);
+uint64_t vc_transcript_words(const vc_circuit *c, uint32_t layer);  /* 7*s+1; 0 if layer >= d */
+uint64_t vc_total_transcript_words(const vc_circuit *c);
+uint32_t vc_depth(const vc_circuit *c);
+uint32_t vc_log_size(const vc_circuit *c, uint32_t layer);           /* layer = d gives log_input */
+
+/* Debug / test helpers (synchronise the stream they are given). */
+/* copies (z[0..63], claim, counter) of the proof state to the host */
+int vc_debug_state(const vc_circuit *c, uint64_t *h_z64, uint64_t *h_claim, uint64_t *h_ctr, void *cuda_stream);
+/* copies value table V_layer (layer = d: the input copy) to the host */
+int vc_debug_values(const vc_circuit *c, uint32_t layer, uint64_t *h_values, void *cuda_stream);
+/* sticky device-side status: 0 = fine, 1 = a non-canonical input word was seen by vc_evaluate */
+int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
+/* number of kernels this library has launched since load (for bench.py's gpu_launches) */
+uint64_t vc_launch_count(void);
+/* selects the kernel schedule: 0 = auto (default), see DESIGN.md "Schedules" for the others */
+int vc_set_schedule(vc_circuit *c, int schedule);
+
+/* Field/PRNG probes for the GPU unit tests: out[i] = op(a[i], b[i]) on the device, n words each,
+ * all DEVICE pointers.  op: 0 add, 1 sub, 2 mul, 3 draw(seed=a[i], ctr=b[i]). */
+int vc_debug_fieldop(int op, const uint64_t *d_a, const uint64_t *d_b, uint64_t *d_out, uint64_t n,
+                     void *cuda_stream);
+/* Integer-multiply roofline microbenchmark: runs `iters` dependent fp61 multiplies in each of `ilp`
+ * independent chains per thread on grid x block threads; d_out receives one word per thread. */
+int vc_bench_modmul(uint32_t grid, uint32_t block, uint32_t iters, uint32_t ilp, uint64_t *d_out, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VC_H */

@@ -1,0 +1,351 @@
+// vc_api.cu — host side of libvc.so: load / evaluate / prove_layer (streaming schedule) / helpers.
+// C ABI documented in include/vc.h.  PyTorch is not involved here: plain CUDA runtime, caller's stream.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "vc_circuit.hpp"
+#include "vc_kernels.cuh"
+#include "vc_line.cuh"
+#include "vc_round.cuh"
+
+namespace vc {
+std::atomic<uint64_t> g_launches{0};
+}
+
+#define VC_LAUNCH(kern, grid, block, smem, stream, ...)                     \
+    do {                                                                    \
+        kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);           \
+        vc::g_launches.fetch_add(1, std::memory_order_relaxed);            \
+    } while (0)
+
+#define CUDA_TRY(x)                                          \
+    do {                                                     \
+        cudaError_t e_ = (x);                                \
+        if (e_ != cudaSuccess) {                             \
+            (void)cudaGetLastError();                        \
+            return e_ == cudaErrorMemoryAllocation ? VC_ERR_NOMEM : VC_ERR_CUDA; \
+        }                                                    \
+    } while (0)
+
+static inline uint32_t grid_for(uint64_t n, int sm_count, int per_thread = 4) {
+    uint64_t b = (n + (uint64_t)vc::RED_BLOCK * per_thread - 1) / ((uint64_t)vc::RED_BLOCK * per_thread);
+    uint64_t cap = (uint64_t)sm_count * 4;
+    if (b < 1) b = 1;
+    if (b > cap) b = cap;
+    return (uint32_t)b;
+}
+
+static uint64_t host_pow(uint64_t a, uint64_t e) {
+    uint64_t r = 1;
+    while (e) { if (e & 1) r = fp61::mul(r, a); a = fp61::mul(a, a); e >>= 1; }
+    return r;
+}
+
+extern "C" const char *vc_strerror(int code) {
+    switch (code) {
+    case VC_OK: return "ok";
+    case VC_ERR_ARG: return "bad argument";
+    case VC_ERR_SHAPE: return "bad circuit shape (non power of two, index out of range, unknown gate type, or a layer below of size 1)";
+    case VC_ERR_STATE: return "call out of order (vc_evaluate, then vc_prove_layer 0..d-1 with one seed)";
+    case VC_ERR_CUDA: return "CUDA error (no device, launch or copy failure)";
+    case VC_ERR_NOMEM: return "out of memory";
+    default: return "unknown error";
+    }
+}
+
+extern "C" void vc_circuit_free(vc_circuit *c) {
+    if (!c) return;
+    for (auto p : c->d_type) cudaFree(p);
+    for (auto p : c->d_in1) cudaFree(p);
+    for (auto p : c->d_in2) cudaFree(p);
+    for (auto p : c->d_V) cudaFree(p);
+    cudaFree(c->d_P); cudaFree(c->d_T0); cudaFree(c->d_T1); cudaFree(c->d_part); cudaFree(c->d_tr);
+    cudaFree(c->d_state);
+    if (c->h_pin) cudaFreeHost(c->h_pin);
+    delete c;
+}
+
+static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit *c) {
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&c->coop_ok, cudaDevAttrCooperativeLaunch, dev));
+    c->d = d; c->log_input = log_input;
+    c->logs.resize(d + 1);
+    for (uint32_t i = 0; i < d; i++) c->logs[i] = layers[i].log_size;
+    c->logs[d] = log_input;
+    for (uint32_t i = 0; i <= d; i++) if (c->logs[i] > 30) return VC_ERR_SHAPE;
+    for (uint32_t i = 1; i <= d; i++) if (c->logs[i] == 0) return VC_ERR_SHAPE;   // a layer below of size 1
+    c->h_type.resize(d); c->h_in1.resize(d); c->h_in2.resize(d); c->wiring.assign(d, 0);
+    uint64_t max_gates = 1, max_tab = 2, total = 0;
+    size_t part = (size_t)vc::MAX_PART_BLOCKS * 3;
+    for (uint32_t i = 0; i < d; i++) {
+        const vc_layer &L = layers[i];
+        if (!L.type || !L.in1 || !L.in2) return VC_ERR_ARG;
+        const uint64_t n = 1ull << L.log_size, nb = 1ull << c->logs[i + 1];
+        bool tree = true, onetype = true;
+        for (uint64_t g = 0; g < n; g++) {
+            if (L.type[g] > 3 || L.in1[g] >= nb || L.in2[g] >= nb) return VC_ERR_SHAPE;
+            tree = tree && L.in1[g] == 2 * g && L.in2[g] == 2 * g + 1;
+            onetype = onetype && L.type[g] == L.type[0];
+        }
+        c->wiring[i] = (tree ? 1u : 0u) | (onetype ? 2u : 0u);
+        c->h_type[i].assign(L.type, L.type + n);
+        c->h_in1[i].assign(L.in1, L.in1 + n);
+        c->h_in2[i].assign(L.in2, L.in2 + n);
+        max_gates = std::max(max_gates, n);
+        max_tab = std::max(max_tab, nb);
+        const uint32_t s = c->logs[i + 1];
+        total += 7ull * s + 1;
+        const uint32_t used = std::min<uint32_t>(s, vc::LINE_NT + vc::LINE_TB);
+        part = std::max(part, (size_t)(1ull << (s - used)) * (s > 1 ? s - 1 : 1));
+    }
+    c->total_words = total;
+    c->part_words = part;
+    c->d_type.assign(d, nullptr); c->d_in1.assign(d, nullptr); c->d_in2.assign(d, nullptr);
+    c->d_V.assign(d + 1, nullptr);
+    for (uint32_t i = 0; i < d; i++) {
+        const size_t n = (size_t)1 << c->logs[i];
+        CUDA_TRY(cudaMalloc(&c->d_type[i], n));
+        CUDA_TRY(cudaMalloc(&c->d_in1[i], n * 4));
+        CUDA_TRY(cudaMalloc(&c->d_in2[i], n * 4));
+        CUDA_TRY(cudaMemcpy(c->d_type[i], layers[i].type, n, cudaMemcpyHostToDevice));
+        CUDA_TRY(cudaMemcpy(c->d_in1[i], layers[i].in1, n * 4, cudaMemcpyHostToDevice));
+        CUDA_TRY(cudaMemcpy(c->d_in2[i], layers[i].in2, n * 4, cudaMemcpyHostToDevice));
+    }
+    for (uint32_t i = 0; i <= d; i++) CUDA_TRY(cudaMalloc(&c->d_V[i], (size_t)8 << c->logs[i]));
+    CUDA_TRY(cudaMalloc(&c->d_P, max_gates * 8));
+    CUDA_TRY(cudaMalloc(&c->d_T0, std::max<uint64_t>(max_tab / 2, 2) * 8));
+    CUDA_TRY(cudaMalloc(&c->d_T1, std::max<uint64_t>(max_tab / 4, 2) * 8));
+    CUDA_TRY(cudaMalloc(&c->d_part, part * 8));
+    CUDA_TRY(cudaMalloc(&c->d_tr, total * 8));
+    CUDA_TRY(cudaMalloc(&c->d_state, sizeof(vc::DevState)));
+    const size_t pin_words = ((size_t)1 << log_input) + ((size_t)1 << c->logs[0]) + total;
+    CUDA_TRY(cudaMallocHost(&c->h_pin, pin_words * 8));
+    // proof state: zero, plus 1/k! for the Lagrange denominators (constants of the method, not data)
+    vc::DevState *hs = new (std::nothrow) vc::DevState();
+    if (!hs) return VC_ERR_NOMEM;
+    std::memset(hs, 0, sizeof(*hs));
+    uint64_t fact = 1;
+    for (uint32_t k = 1; k <= vc::MAX_VARS; k++) fact = fp61::mul(fact, k);
+    uint64_t inv = host_pow(fact, fp61::P - 2);
+    for (int k = vc::MAX_VARS; k >= 0; k--) { hs->invfact[k] = inv; inv = fp61::mul(inv, (uint64_t)k); }
+    cudaError_t e = cudaMemcpy(c->d_state, hs, sizeof(*hs), cudaMemcpyHostToDevice);
+    delete hs;
+    CUDA_TRY(e);
+    CUDA_TRY(cudaFuncSetAttribute(vc::k_line, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    return vc::fused_init(c);
+}
+
+extern "C" int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit **out) {
+    if (!layers || !out || d == 0) return VC_ERR_ARG;
+    *out = nullptr;
+    vc_circuit *c = new (std::nothrow) vc_circuit();
+    if (!c) return VC_ERR_NOMEM;
+    int rc;
+    try { rc = load_impl(layers, d, log_input, c); } catch (const std::bad_alloc &) { rc = VC_ERR_NOMEM; }
+    if (rc != VC_OK) { vc_circuit_free(c); return rc; }
+    *out = c;
+    return VC_OK;
+}
+
+// ------------------------------------------------------------------ a1
+extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, void *cuda_stream) {
+    if (!c || !d_input) return VC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint32_t d = c->d;
+    const uint64_t n_in = 1ull << c->log_input;
+    VC_LAUNCH(vc::k_copy_input, grid_for(n_in, c->sm_count), vc::RED_BLOCK, 0, st, d_input, c->d_V[d], n_in, c->d_state);
+    for (int i = (int)d - 1; i >= 0; i--) {
+        const uint32_t n = 1u << c->logs[i];
+        VC_LAUNCH(vc::k_eval, grid_for(n, c->sm_count, 2), vc::RED_BLOCK, 0, st, c->d_type[i], c->d_in1[i], c->d_in2[i],
+                  c->d_V[i + 1], c->d_V[i], (i == 0 ? d_outputs : (uint64_t *)nullptr), n);
+    }
+    CUDA_TRY(cudaGetLastError());
+    c->next_layer = 0;
+    return VC_OK;
+}
+
+// ------------------------------------------------------------------ a2-a7, streaming schedule
+int vc::enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {
+    const uint32_t si = c->logs[layer], s = c->logs[layer + 1];
+    const uint32_t n = 1u << si;
+    vc::DevState *S = c->d_state;
+    const uint8_t *type = c->d_type[layer];
+    const uint32_t *in1 = c->d_in1[layer], *in2 = c->d_in2[layer];
+    const uint64_t *Vb = c->d_V[layer + 1];
+    const uint32_t gg = grid_for(n, c->sm_count);
+    const uint32_t cb = si < (uint32_t)vc::BETA_LOG_CHUNK ? si : (uint32_t)vc::BETA_LOG_CHUNK;
+    if (layer == 0) VC_LAUNCH(vc::k_start, 1, 64, 0, st, S, seed, si);
+    VC_LAUNCH(vc::k_beta, 1u << (si - cb), 256, 0, st, S, c->d_P, si);
+    if (layer == 0) VC_LAUNCH(vc::k_dot_claim, gg, vc::RED_BLOCK, 0, st, c->d_P, c->d_V[0], n, c->d_part, S);
+    uint64_t *tr = d_tr;
+    for (int phase = 1; phase <= 2; phase++) {
+        const uint64_t *tab = Vb;
+        for (uint32_t j = 0; j < s; j++) {
+            uint64_t *out = (j & 1) ? c->d_T1 : c->d_T0;
+            const uint32_t half = 1u << (s - j - 1);
+            const uint32_t gu = grid_for(std::max(n, half), c->sm_count);
+            if (phase == 1) {
+                VC_LAUNCH(vc::k_round<1>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
+                VC_LAUNCH(vc::k_update<1>, gu, vc::RED_BLOCK, 0, st, in1, c->d_P, tab, out, S, j, n, half);
+            } else {
+                VC_LAUNCH(vc::k_round<2>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
+                VC_LAUNCH(vc::k_update<2>, gu, vc::RED_BLOCK, 0, st, in2, c->d_P, tab, out, S, j, n, half);
+            }
+            tab = out;
+            tr += 3;
+        }
+    }
+    const uint32_t used = std::min<uint32_t>(s, vc::LINE_NT + vc::LINE_TB);
+    VC_LAUNCH(vc::k_line, 1u << (s - used), 256, vc::line_smem_words(s) * 8, st, Vb, s, S, c->d_part, tr);
+    return cudaGetLastError() == cudaSuccess ? VC_OK : VC_ERR_CUDA;
+}
+
+extern "C" int vc_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_transcript, uint64_t cap_words,
+                              void *cuda_stream) {
+    if (!c || !d_transcript) return VC_ERR_ARG;
+    if (layer >= c->d) return VC_ERR_ARG;
+    if (c->next_layer < 0 || (uint32_t)c->next_layer != layer) return VC_ERR_STATE;
+    if (layer > 0 && seed != c->seed) return VC_ERR_STATE;
+    if (cap_words < 7ull * c->logs[layer + 1] + 1) return VC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc;
+    if (c->schedule != 1 && vc::fused_supported(c, layer)) rc = vc::enqueue_layer_fused(c, layer, seed, d_transcript, st);
+    else rc = vc::enqueue_layer_streaming(c, layer, seed, d_transcript, st);
+    if (rc != VC_OK) return rc;
+    c->seed = seed;
+    c->next_layer = (int)layer + 1;
+    return VC_OK;
+}
+
+extern "C" int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, uint64_t cap_words, void *cuda_stream) {
+    if (!c || !d_transcript) return VC_ERR_ARG;
+    if (cap_words < c->total_words) return VC_ERR_ARG;
+    if (c->next_layer != 0) return VC_ERR_STATE;
+    uint64_t w = 0;
+    for (uint32_t i = 0; i < c->d; i++) {
+        const uint64_t nw = 7ull * c->logs[i + 1] + 1;
+        int rc = vc_prove_layer(c, i, seed, d_transcript + w, nw, cuda_stream);
+        if (rc != VC_OK) return rc;
+        w += nw;
+    }
+    return VC_OK;
+}
+
+extern "C" int vc_run_host(vc_circuit *c, const uint64_t *h_input, uint64_t seed, uint64_t *h_outputs,
+                           uint64_t *h_transcript, uint64_t cap_words, void *cuda_stream) {
+    if (!c || !h_input || !h_outputs || !h_transcript) return VC_ERR_ARG;
+    if (cap_words < c->total_words) return VC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n_in = (size_t)1 << c->log_input, n_out = (size_t)1 << c->logs[0];
+    // H2D straight into the handle's own input table V_d; vc_evaluate then checks it in place
+    CUDA_TRY(cudaMemcpyAsync(c->d_V[c->d], h_input, n_in * 8, cudaMemcpyHostToDevice, st));
+    int rc = vc_evaluate(c, c->d_V[c->d], nullptr, cuda_stream);
+    if (rc == VC_OK) rc = vc_prove(c, seed, c->d_tr, c->total_words, cuda_stream);
+    if (rc != VC_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h_outputs, c->d_V[0], n_out * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h_transcript, c->d_tr, c->total_words * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    uint32_t flags = 0;
+    CUDA_TRY(cudaMemcpy(&flags, &c->d_state->flags, 4, cudaMemcpyDeviceToHost));
+    return (flags & 1u) ? VC_ERR_ARG : VC_OK;
+}
+
+// ------------------------------------------------------------------ sizes, debug, probes
+extern "C" uint64_t vc_transcript_words(const vc_circuit *c, uint32_t layer) {
+    return (c && layer < c->d) ? 7ull * c->logs[layer + 1] + 1 : 0;
+}
+extern "C" uint64_t vc_total_transcript_words(const vc_circuit *c) { return c ? c->total_words : 0; }
+extern "C" uint32_t vc_depth(const vc_circuit *c) { return c ? c->d : 0; }
+extern "C" uint32_t vc_log_size(const vc_circuit *c, uint32_t layer) { return (c && layer <= c->d) ? c->logs[layer] : 0; }
+extern "C" uint64_t vc_launch_count(void) { return vc::g_launches.load(); }
+
+extern "C" int vc_set_schedule(vc_circuit *c, int schedule) {
+    if (!c || schedule < 0 || schedule > 1) return VC_ERR_ARG;
+    c->schedule = schedule;
+    return VC_OK;
+}
+
+extern "C" int vc_debug_state(const vc_circuit *c, uint64_t *h_z64, uint64_t *h_claim, uint64_t *h_ctr, void *cuda_stream) {
+    if (!c) return VC_ERR_ARG;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    vc::DevState hs;
+    CUDA_TRY(cudaMemcpy(&hs, c->d_state, sizeof(hs), cudaMemcpyDeviceToHost));
+    if (h_z64) std::memcpy(h_z64, hs.z, sizeof(hs.z));
+    if (h_claim) *h_claim = hs.claim;
+    if (h_ctr) *h_ctr = hs.ctr;
+    return VC_OK;
+}
+
+extern "C" int vc_debug_values(const vc_circuit *c, uint32_t layer, uint64_t *h_values, void *cuda_stream) {
+    if (!c || !h_values || layer > c->d) return VC_ERR_ARG;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    CUDA_TRY(cudaMemcpy(h_values, c->d_V[layer], (size_t)8 << c->logs[layer], cudaMemcpyDeviceToHost));
+    return VC_OK;
+}
+
+extern "C" int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream) {
+    if (!c || !h_flags) return VC_ERR_ARG;
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    CUDA_TRY(cudaMemcpy(h_flags, &c->d_state->flags, 4, cudaMemcpyDeviceToHost));
+    return VC_OK;
+}
+
+namespace vc {
+__global__ void k_fieldop(int op, const uint64_t *a, const uint64_t *b, uint64_t *out, uint64_t n) {
+    for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        uint64_t x = a[i], y = b[i], r;
+        if (op == 0) r = fp61::add(x, y);
+        else if (op == 1) r = fp61::sub(x, y);
+        else if (op == 2) r = fp61::mul(x, y);
+        else if (op == 3) r = fp61::draw(x, y);
+        else { acc128 acc; acc.clear(); for (int k = 0; k < 64; k++) acc.mac(x, y); r = acc.value(); }  // 64 x*y, lazily
+        out[i] = r;
+    }
+}
+// ILP independent dependent-chains of fp61 multiplies per thread: the integer-multiply roofline probe
+template <int ILP>
+__global__ void k_bench_modmul(uint32_t iters, uint64_t *out) {
+    uint64_t x[ILP];
+    const uint64_t tid = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < ILP; k++) x[k] = fp61::draw(tid, k) | 1;
+    const uint64_t m = fp61::draw(12345, tid);
+    for (uint32_t i = 0; i < iters; i++) {
+#pragma unroll
+        for (int k = 0; k < ILP; k++) x[k] = fp61::mul(x[k], m);
+    }
+    uint64_t r = 0;
+#pragma unroll
+    for (int k = 0; k < ILP; k++) r = fp61::add(r, x[k]);
+    out[tid] = r;
+}
+}  // namespace vc
+
+extern "C" int vc_debug_fieldop(int op, const uint64_t *d_a, const uint64_t *d_b, uint64_t *d_out, uint64_t n,
+                                void *cuda_stream) {
+    if (!d_a || !d_b || !d_out || op < 0 || op > 4) return VC_ERR_ARG;
+    if (n == 0) return VC_OK;
+    VC_LAUNCH(vc::k_fieldop, (uint32_t)std::min<uint64_t>((n + 255) / 256, 1184), 256, 0, (cudaStream_t)cuda_stream, op, d_a, d_b, d_out, n);
+    CUDA_TRY(cudaGetLastError());
+    return VC_OK;
+}
+
+extern "C" int vc_bench_modmul(uint32_t grid, uint32_t block, uint32_t iters, uint32_t ilp, uint64_t *d_out, void *cuda_stream) {
+    if (!d_out || grid == 0 || block == 0 || block > 1024) return VC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    switch (ilp) {
+    case 1: VC_LAUNCH(vc::k_bench_modmul<1>, grid, block, 0, st, iters, d_out); break;
+    case 2: VC_LAUNCH(vc::k_bench_modmul<2>, grid, block, 0, st, iters, d_out); break;
+    case 4: VC_LAUNCH(vc::k_bench_modmul<4>, grid, block, 0, st, iters, d_out); break;
+    case 8: VC_LAUNCH(vc::k_bench_modmul<8>, grid, block, 0, st, iters, d_out); break;
+    default: return VC_ERR_ARG;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return VC_OK;
+}

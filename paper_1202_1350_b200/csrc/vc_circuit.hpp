@@ -1,0 +1,49 @@
+// vc_circuit.hpp — the opaque handle behind include/vc.h (host side).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <vector>
+
+#include "../../include/vc.h"
+#include "vc_state.cuh"
+
+struct vc_circuit {
+    uint32_t d = 0, log_input = 0;
+    std::vector<uint32_t> logs;                 // logs[i] = log2 size of layer i, i = 0..d (d = input)
+    // host copies of the records (the verifier runs on the host)
+    std::vector<std::vector<uint8_t>> h_type;
+    std::vector<std::vector<uint32_t>> h_in1, h_in2;
+    // device: records (SoA), value tables
+    std::vector<uint8_t *> d_type;
+    std::vector<uint32_t *> d_in1, d_in2;
+    std::vector<uint64_t *> d_V;                // d+1 tables, V[d] = input copy
+    // per-layer wiring class (set at load): bit 0 = "tree" (in1 = 2g, in2 = 2g+1), bit 1 = single type
+    std::vector<uint32_t> wiring;
+    // scratch
+    uint64_t *d_P = nullptr;                    // weights, max layer size
+    uint64_t *d_T0 = nullptr, *d_T1 = nullptr;  // fold ping-pong
+    uint64_t *d_part = nullptr;                 // block partials
+    uint64_t *d_tr = nullptr;                   // internal transcript buffer (vc_run_host)
+    vc::DevState *d_state = nullptr;
+    uint64_t *h_pin = nullptr;                  // pinned staging for vc_run_host
+    size_t part_words = 0;
+    uint64_t total_words = 0;
+    // proof sequencing
+    int next_layer = -1;                        // -1: vc_evaluate not called yet
+    uint64_t seed = 0;
+    int schedule = 0;
+    int sm_count = 148;
+    int coop_ok = 0;
+
+    uint32_t log_below(uint32_t i) const { return logs[i + 1]; }
+};
+
+namespace vc {
+extern std::atomic<uint64_t> g_launches;
+int enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
+int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);  // vc_fused.cu
+int fused_supported(const vc_circuit *c, uint32_t layer);
+int fused_init(vc_circuit *c);
+}  // namespace vc

@@ -1,0 +1,251 @@
+"""GPU parity: the CUDA path (through the C ABI of libvc.so) vs the CPU oracle, word for word.
+
+All arithmetic is integer, so the bar is bit-exact (BASELINE.json north_star).  Inputs come from
+vc_workloads (seeded); expected values come from oracle/ or from tests/golden/*.txt, which
+tests/golden/make_golden.py wrote from the oracle alone.
+"""
+import hashlib
+import os
+import random
+
+import numpy as np
+import pytest
+
+import oracle
+import vc_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+P = (1 << 61) - 1
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def vc():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1202_1350_b200 as v
+    v.lib()                       # fails loudly if libvc.so is missing
+    return v
+
+
+def _sha(a):
+    return hashlib.sha256(np.ascontiguousarray(a, dtype="<u8").tobytes()).hexdigest()
+
+
+def _golden(k):
+    g = {"layers": {}}
+    with open(os.path.join(GOLDEN, f"config{k}.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            p = line.split()
+            if p[0] == "layer":
+                g["layers"][int(p[1])] = (int(p[2]), p[3], int(p[4]), int(p[5]))
+            else:
+                g[p[0]] = p[1]
+    return g
+
+
+def _gpu_prove(vc, c, seed, schedule=0, layerwise=False):
+    gc = vc.Circuit(c)
+    gc.set_schedule(schedule)
+    gc.set_input(c.input)
+    gc.evaluate()
+    if layerwise:
+        gc.prove_layerwise(seed)
+    else:
+        gc.prove(seed)
+    out, tr = gc.outputs().copy(), gc.transcript().copy()
+    assert gc.flags() == 0
+    return gc, out, tr
+
+
+# ------------------------------------------------------------------ field arithmetic on the device
+def test_device_field_ops_and_draws(vc):
+    import torch
+    rnd = random.Random(1)
+    edge = [0, 1, 2, P - 1, P - 2, 1 << 60, (1 << 60) + 1, (1 << 32) - 1, 1 << 32, 12345678901234567]
+    a = edge * len(edge) + [rnd.randrange(P) for _ in range(5000)]
+    b = [y for y in edge for _ in edge] + [rnd.randrange(P) for _ in range(5000)]
+    ta = torch.from_numpy(np.array(a, dtype=np.uint64).view(np.int64)).cuda()
+    tb = torch.from_numpy(np.array(b, dtype=np.uint64).view(np.int64)).cuda()
+    to = torch.empty_like(ta)
+    L = vc.lib()
+    for op, fn in [(0, lambda x, y: (x + y) % P), (1, lambda x, y: (x - y) % P), (2, lambda x, y: x * y % P),
+                   (4, lambda x, y: 64 * x * y % P)]:
+        assert L.vc_debug_fieldop(op, ta.data_ptr(), tb.data_ptr(), to.data_ptr(), ta.numel(), 0) == 0
+        got = to.cpu().numpy().view(np.uint64)
+        assert [int(v) for v in got] == [fn(x, y) for x, y in zip(a, b)], op
+    seeds = np.array([0, 0, 0, 1234567, 2002, 2002], dtype=np.uint64)
+    ctrs = np.array([0, 1, 2, 0, 5, 999], dtype=np.uint64)
+    ts, tc = (torch.from_numpy(x.view(np.int64)).cuda() for x in (seeds, ctrs))
+    tt = torch.empty_like(ts)
+    assert L.vc_debug_fieldop(3, ts.data_ptr(), tc.data_ptr(), tt.data_ptr(), ts.numel(), 0) == 0
+    got = [int(v) for v in tt.cpu().numpy().view(np.uint64)]
+    assert got == [oracle.draw(int(s), int(k)) for s, k in zip(seeds, ctrs)]
+    assert got[0] == 0xE220A8397B1DCDAF & P        # published splitmix64 vector, low 61 bits
+
+
+# ------------------------------------------------------------------ element-by-element on small/medium circuits
+RANDOM_CASES = [
+    ([0, 1], 1, 1), ([1, 2, 1], 2, 2), ([0, 2, 3], 2, 4), ([3, 1, 2], 3, 5),
+    ([0, 1, 2, 3, 4, 5], 6, 9), ([4, 6, 5], 7, 10), ([6, 3], 5, 12),
+    ([9, 12, 10, 13], 11, 13),          # several tiles of every kernel + ragged sizes between layers
+    ([14, 11, 15], 13, 14),
+]
+
+
+@pytest.mark.parametrize("schedule", [1, 0])
+@pytest.mark.parametrize("log_sizes,log_input,seed", RANDOM_CASES)
+def test_random_circuits_bit_exact(vc, log_sizes, log_input, seed, schedule):
+    c = W.random_circuit(log_sizes, log_input, seed)
+    oc = oracle.OracleCircuit(c)
+    want_out, want_tr, want_z, want_claim = oc.prove(c.input, 500 + seed)
+    gc, out, tr = _gpu_prove(vc, c, 500 + seed, schedule)
+    V = oc.evaluate(c.input)
+    for i in range(c.d + 1):
+        assert np.array_equal(gc.values(i), V[i]), f"value table {i}"
+    assert np.array_equal(out, want_out)
+    bad = np.nonzero(tr != want_tr)[0]
+    assert bad.size == 0, f"first mismatch at word {bad[:5]} of {tr.size}"
+    z, claim, ctr = gc.state()
+    assert claim == want_claim and np.array_equal(z[:c.log_input], want_z[:c.log_input])
+    assert ctr == c.layers[0].log_size + sum(2 * c.log_below(i) + 1 for i in range(c.d))
+    assert gc.verify(c.input, out, 500 + seed, tr) == (True, 0, 0)
+    gc.close()
+
+
+@pytest.mark.parametrize("schedule", [1, 0])
+def test_structured_small_circuits_bit_exact(vc, schedule):
+    for c, seed in [(W.f0_circuit(5, 5), 31), (W.matmul_circuit(3, 6), 32), (W.pm_circuit(6, 2, 7, planted=3), 33),
+                    (W.config(1), W.challenge_seed(1))]:
+        oc = oracle.OracleCircuit(c)
+        want_out, want_tr, _, want_claim = oc.prove(c.input, seed)
+        gc, out, tr = _gpu_prove(vc, c, seed, schedule, layerwise=True)
+        assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), c.name
+        assert gc.state()[1] == want_claim
+        gc.close()
+
+
+# ------------------------------------------------------------------ full sizes: golden digests written by the oracle
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_configs_match_oracle_golden(vc, k):
+    path = os.path.join(GOLDEN, f"config{k}.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet (python tests/golden/make_golden.py {k})")
+    g = _golden(k)
+    c = W.config(k)
+    seed = W.challenge_seed(k)
+    gc, out, tr = _gpu_prove(vc, c, seed)      # the launch configuration bench.py times (schedule 0)
+    assert int(g["gates"]) == c.gates and int(g["transcript_words"]) == tr.size
+    assert _sha(out) == g["outputs_sha256"] and int(out[0]) == int(g["output0"])
+    w = 0
+    for i in range(c.d):
+        n = c.transcript_words(i)
+        s, digest, first, last = g["layers"][i]
+        seg = tr[w:w + n]
+        assert (int(seg[0]), int(seg[-1])) == (first, last), f"config {k} layer {i}"
+        assert _sha(seg) == digest, f"config {k} layer {i}"
+        w += n
+    assert _sha(tr) == g["transcript_sha256"]
+    assert gc.state()[1] == int(g["final_claim"])
+    # properties that hold at any size: both verifiers accept the GPU transcript
+    assert gc.verify(c.input, out, seed, tr) == (True, 0, 0)
+    if k in (1, 2, 4):
+        assert oracle.OracleCircuit(c).verify(c.input, out, seed, tr) == (True, 0, 0)
+    gc.close()
+
+
+def test_sampled_layers_of_config2_against_oracle_in_isolation(vc):
+    """Full-size config 2 in the bench launch configuration; the oracle re-proves sampled layers one by one."""
+    c = W.config(2)
+    seed = W.challenge_seed(2)
+    gc, out, tr = _gpu_prove(vc, c, seed)
+    oc = oracle.OracleCircuit(c)
+    V = oc.evaluate(c.input)
+    offs = np.cumsum([0] + [c.transcript_words(i) for i in range(c.d)])
+    for i in (0, 7, 13, 17):
+        z, claim, ctr = oc.layer_entry(i, seed, V[i])
+        want, *_ = oc.prove_layer(i, V[i + 1], seed, ctr, z, claim, debug=False)
+        assert np.array_equal(tr[offs[i]:offs[i + 1]], want), f"layer {i}"
+    gc.close()
+
+
+# ------------------------------------------------------------------ verifier of the library: tamper = fault injection
+def test_library_verifier_rejects_tampering(vc):
+    c = W.random_circuit([1, 2, 3, 2], 3, 61)
+    seed = 808
+    gc, out, tr = _gpu_prove(vc, c, seed)
+    oc = oracle.OracleCircuit(c)
+    assert gc.verify(c.input, out, seed, tr) == (True, 0, 0)
+    for w in range(tr.size):
+        bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+        got = gc.verify(c.input, out, seed, bad)
+        assert got == oc.verify(c.input, out, seed, bad) and not got[0], w
+    for k in range(out.size):
+        bad = out.copy(); bad[k] = (int(bad[k]) + 1) % P
+        assert gc.verify(c.input, bad, seed, tr) == (False, 0, 0)
+    for k in range(c.input.size):
+        bad = c.input.copy(); bad[k] = (int(bad[k]) + 1) % P
+        assert gc.verify(bad, out, seed, tr) == (False, c.d, 0)
+    gc.close()
+
+
+# ------------------------------------------------------------------ boundary behaviour
+def test_call_order_and_argument_errors(vc):
+    import torch
+    c = W.random_circuit([1, 2], 2, 3)
+    gc = vc.Circuit(c)
+    gc.set_input(c.input)
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_prove_layer(gc.handle, 0, 1, gc.d_transcript)      # before vc_evaluate
+    assert e.value.code == vc.VC_ERR_STATE
+    gc.evaluate()
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_prove_layer(gc.handle, 1, 1, gc.d_transcript)      # out of order
+    assert e.value.code == vc.VC_ERR_STATE
+    small = torch.zeros(3, dtype=torch.int64, device="cuda")
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_prove_layer(gc.handle, 0, 1, small)                # capacity
+    assert e.value.code == vc.VC_ERR_ARG
+    vc.vc_prove_layer(gc.handle, 0, 1, gc.d_transcript)
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_prove_layer(gc.handle, 1, 2, gc.d_transcript)      # seed changed mid-proof
+    assert e.value.code == vc.VC_ERR_STATE
+    gc.close()
+    bad = W.random_circuit([1, 2], 2, 3)
+    bad.layers[0].in1[0] = 99
+    with pytest.raises(vc.VCError) as e:
+        vc.Circuit(bad)
+    assert e.value.code == vc.VC_ERR_SHAPE
+    bad = W.random_circuit([1, 0], 2, 3)                          # a layer below of size 1
+    with pytest.raises(vc.VCError) as e:
+        vc.Circuit(bad)
+    assert e.value.code == vc.VC_ERR_SHAPE
+
+
+def test_non_canonical_input_is_flagged(vc):
+    c = W.random_circuit([1, 2], 2, 3)
+    gc = vc.Circuit(c)
+    x = c.input.copy(); x[1] = np.uint64(P)
+    gc.set_input(x)
+    gc.evaluate()
+    assert gc.flags() & 1
+    gc.close()
+
+
+def test_run_host_end_to_end_matches(vc):
+    import torch
+    c = W.config(1)
+    seed = W.challenge_seed(1)
+    want_out, want_tr, _, _ = oracle.OracleCircuit(c).prove(c.input, seed)
+    gc = vc.Circuit(c)
+    h_in = torch.from_numpy(c.input.view(np.int64)).pin_memory()
+    h_out = torch.zeros(gc.n_out, dtype=torch.int64).pin_memory()
+    h_tr = torch.zeros(gc.words, dtype=torch.int64).pin_memory()
+    for _ in range(2):           # twice: the handle is reusable
+        vc.vc_run_host(gc.handle, h_in, seed, h_out, h_tr)
+        assert np.array_equal(h_out.numpy().view(np.uint64), want_out)
+        assert np.array_equal(h_tr.numpy().view(np.uint64), want_tr)
+    gc.close()
