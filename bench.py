@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py — GKR prover gates/s (all layers, device-timed) on BASELINE.json's configs, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference] [--schedule s]
+
+A "step" is one pass of the whole hot path (vc_evaluate + vc_prove_layer for every layer)
+over one synthetic input that is already resident in HBM.  N=1 workload: BASELINE.json configs[1]
+(F2 circuit, n = 2^20).  N>1: replicas only: every rank proves its own instance of the
+same circuit (data seed + rank), no data-path collective; value = gates of all ranks / max-over-ranks time.
+See DESIGN.md "Measurement" for the algorithmic byte / multiply counts used in the roofline objects.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import vc_workloads as W  # noqa: E402
+
+METRIC = "GKR prover gates/sec (all layers, device-timed)"
+UNIT = "gates/s"
+
+
+# ---------------------------------------------------------------------------------------------- counts
+def algorithmic_counts(c):
+    """Algorithmic bytes and mod-p multiplies of one step, from SURVEY.md §8(d).
+
+    per gate-round: 9 B record + 16 B weight read+write + 8 B fixed operand (phase 1 only) -> 33 B / 25 B;
+    per layer: two shrinking fold tables (read 8*2^(s-j), write half: ~24*2^s B per phase), one 8*2^s B pass for
+    the line restriction, 8*2^{s_i} B to write the beta weights; evaluation: 9 B record + 16 B operands + 8 B result.
+    multiplies: 3 per gate-round, 2^{s_i} (beta), ~2*2^s (folds), (s-1)*2^s (line), 1 per MULT gate (evaluation).
+    """
+    per_layer = []
+    for i, L in enumerate(c.layers):
+        n, s = 1 << L.log_size, c.log_below(i)
+        nb = 1 << s
+        rounds_bytes = n * s * (33 + 25)
+        table_bytes = 2 * 24 * nb
+        line_bytes = 8 * nb
+        beta_bytes = 8 * n
+        eval_bytes = n * 33
+        mm = 3 * n * 2 * s + n + 2 * nb + max(s - 1, 0) * nb
+        mm_eval = int(np.count_nonzero(L.type == W.MULT))
+        per_layer.append(dict(n=n, s=s, prove_bytes=rounds_bytes + table_bytes + line_bytes + beta_bytes,
+                              round_bytes=[n * (17 + (8 if ph == 1 else 0)) + 8 * (nb >> j) for ph in (1, 2) for j in range(s)],
+                              eval_bytes=eval_bytes, modmul=mm + mm_eval))
+    return dict(layers=per_layer,
+                bytes=sum(l["prove_bytes"] + l["eval_bytes"] for l in per_layer),
+                modmul=sum(l["modmul"] for l in per_layer))
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([p.strip() for p in out.split(",")])
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        self.stop_flag.set()
+        self.join(timeout=6)
+        sm = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
+        mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for s in self.samples for n, v in zip(names, s[2:6]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------- oracle legs
+def oracle_full_proof(k: int):
+    """The oracle as it stands, one thread, whole proof of config k. Returns (seconds, gates)."""
+    import oracle
+    c = W.config(k)
+    oc = oracle.OracleCircuit(c)
+    t0 = time.perf_counter()
+    oc.prove(c.input, W.challenge_seed(k))
+    return time.perf_counter() - t0, c.gates
+
+
+def oracle_sample_step(oc, c, V, seed, layers):
+    """Oracle proves the sampled layers in isolation (entry state from the counter-based draws)."""
+    import oracle  # noqa: F401
+    gr = 0
+    for i in layers:
+        z, claim, ctr = oc.layer_entry(i, seed, V[i])
+        oc.prove_layer(i, V[i + 1], seed, ctr, z, claim, debug=False)
+        gr += (1 << c.layers[i].log_size) * 2 * c.log_below(i)
+    return gr
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores (rank 0 only), bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    k = args.config
+    c = W.config(k)
+    seed = W.challenge_seed(k)
+    oc = oracle.OracleCircuit(c)
+    # sample: the layers whose gate-rounds sum to ~5 M (about a second of oracle time), widest first that fits
+    order = sorted(range(c.d), key=lambda i: -(1 << c.layers[i].log_size) * c.log_below(i))
+    budget, layers, tot = 6_000_000, [], 0
+    for i in order:
+        gr = (1 << c.layers[i].log_size) * 2 * c.log_below(i)
+        if tot + gr <= budget:
+            layers.append(i)
+            tot += gr
+    layers = sorted(layers) or [c.d - 1 if c.gate_rounds < budget else 0]
+    V = oc.evaluate(c.input)
+    for _ in range(args.warmup):
+        oracle_sample_step(oc, c, V, seed, layers)
+    t0 = time.perf_counter()
+    gr = 0
+    for _ in range(args.steps):
+        V = oc.evaluate(c.input)
+        gr += oracle_sample_step(oc, c, V, seed, layers)
+    dt = (time.perf_counter() - t0) / args.steps
+    gr //= args.steps
+    full = dt * c.gate_rounds / gr                       # oracle time is ~proportional to gate-rounds
+    value = c.gates / full
+    sample = (f"per step: evaluate + oracle proof of layers {layers[0]}..{layers[-1]} ({len(layers)} layers, {gr} of "
+              f"{c.gate_rounds} gate-rounds) in isolation; whole-proof time extrapolated by gate-rounds")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}", "gates": c.gates},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import ctypes as C
+    import paper_1202_1350_b200 as vc
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    k = args.config
+    c = W.config(k)
+    if rank > 0:                                   # replicas: same circuit, another seeded input of the same recipe
+        c.input = np.random.default_rng(W.data_seed(k) + rank).permutation(c.input)
+    seed = W.challenge_seed(k)
+    L = vc.lib()
+    gc = vc.Circuit(c)
+    gc.set_schedule(args.schedule)
+    gc.set_input(c.input)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        gc.evaluate(stream)
+        gc.prove(seed, stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    # ---- device-timed steps, inputs resident; L2 flushed between steps outside the event pairs
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = L.vc_launch_count()
+    barrier()
+    for a, b in evs:
+        flush.fill_(1)
+        a.record(stream)
+        step()
+        b.record(stream)
+    barrier()
+    launches = int(L.vc_launch_count() - l0)
+    ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(ms))
+    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
+    h_in = torch.from_numpy(np.ascontiguousarray(c.input).view(np.int64)).pin_memory()
+    h_out = torch.zeros(gc.n_out, dtype=torch.int64).pin_memory()
+    h_tr = torch.zeros(gc.words, dtype=torch.int64).pin_memory()
+    for _ in range(2):
+        vc.vc_run_host(gc.handle, h_in, seed, h_out, h_tr, stream)
+    barrier()
+    e2e_ms = 0.0
+    for _ in range(args.steps):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        vc.vc_run_host(gc.handle, h_in, seed, h_out, h_tr, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        e2e_ms += a.elapsed_time(b)
+    barrier()
+    clocks = sampler.summary()
+    if world > 1:
+        t = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = float(t[0]), float(t[1])
+    ms_per_step = total_ms / args.steps
+    value = c.gates * world / (ms_per_step * 1e-3)
+    e2e_value = c.gates * world / (e2e_ms / args.steps * 1e-3)
+
+    if rank == 0:
+        # ---- per-kernel-kind timing (CUDA events inside the library, on the launching stream), one extra step
+        counts = algorithmic_counts(c)
+        peak, peak_src = measured_peaks()
+        L.vc_profile_enable(1)
+        flush.fill_(1)
+        step()
+        nk = 8
+        pl, pm = (C.c_uint64 * nk)(), (C.c_double * nk)()
+        L.vc_profile_read(pl, pm)
+        L.vc_profile_enable(0)
+        kinds = ["evaluate", "setup(beta,start)", "round", "update+fold", "line", "fused_small", "fused_wide", "misc"]
+        prof = {kinds[i]: {"launches": int(pl[i]), "ms": round(float(pm[i]), 4)} for i in range(nk) if pl[i]}
+        prof_total = sum(v["ms"] for v in prof.values())
+        dom = max(prof, key=lambda n: prof[n]["ms"])
+        if dom == "round":
+            dom_bytes = sum(sum(l["round_bytes"]) for l in counts["layers"])
+            dom_desc = "k_round<phase>: per launch n*(9 B record + 8 B weight [+ 8 B operand in phase 1]) + 8*2^(s-j) B table"
+        else:
+            dom_bytes = counts["bytes"] * (prof[dom]["ms"] / prof_total)
+            dom_desc = f"{dom}: share of the step's algorithmic bytes by time"
+        ach = dom_bytes / (prof[dom]["ms"] * 1e-3) / 1e9
+        # integer-multiply rate (fp61 multiplies/s) measured live: 8 independent chains per thread
+        outw = torch.empty(148 * 8 * 256, dtype=torch.int64, device="cuda")
+        best = 0.0
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            L.vc_bench_modmul(148 * 8, 256, 4096, 8, outw.data_ptr(), stream.cuda_stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            best = max(best, 148 * 8 * 256 * 4096 * 8 / (a.elapsed_time(b) * 1e-3))
+        t_hbm = counts["bytes"] / (peak * 1e9)
+        t_alu = counts["modmul"] / best
+        roof_ms = max(t_hbm, t_alu) * 1e3
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": None, "peak_source": peak_src, "what": dom_desc,
+                    "kernel_share_of_step": prof[dom]["ms"] / prof_total, "per_kind": prof,
+                    "step": {"algorithmic_bytes": counts["bytes"], "algorithmic_modmul": counts["modmul"],
+                             "hbm_bound_ms": t_hbm * 1e3, "modmul_rate_per_s": best, "alu_bound_ms": t_alu * 1e3,
+                             "roofline_ms": roof_ms, "frac": roof_ms / ms_per_step,
+                             "frac_at_8TBps": counts["bytes"] / 8e12 * 1e3 / ms_per_step}}
+        # ---- the oracle, timed beside it on the host cores (bounded: one whole proof of config 2 is ~15 s)
+        cpu = None
+        if not args.no_cpu_baseline:
+            if c.gate_rounds <= 200_000_000:
+                sec, gates = oracle_full_proof(k)
+                cpu = {"value": gates / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+                       "sample": f"one whole proof of this workload (evaluate + all {c.d} layers), {sec:.1f} s, 1 thread"}
+            else:
+                import oracle
+                oc = oracle.OracleCircuit(c)
+                V = oc.evaluate(c.input)
+                lay = [max(range(c.d), key=lambda i: (1 << c.layers[i].log_size) * c.log_below(i))]
+                t0 = time.perf_counter()
+                gr = oracle_sample_step(oc, c, V, seed, lay)
+                sec = (time.perf_counter() - t0) * c.gate_rounds / gr
+                cpu = {"value": c.gates / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+                       "sample": f"layer {lay[0]} in isolation ({gr} of {c.gate_rounds} gate-rounds), extrapolated by gate-rounds"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
+                "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}", "gates": c.gates, "layers": c.d,
+                           "rounds": c.rounds, "gate_rounds": c.gate_rounds, "replicas": world,
+                           "schedule": args.schedule, "l2": "flushed between steps (256 MiB fill, outside the event pairs)",
+                           "ms_min": min(ms), "ms_median": float(np.median(ms))},
+                "clocks": clocks, "gpu_launches": launches,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(c.input.nbytes),
+                        "d2h_bytes_per_step": int(8 * (gc.n_out + gc.words)), "ms_per_step": e2e_ms / args.steps},
+                "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    gc.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--schedule", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -13,13 +13,10 @@
 
 namespace vc {
 std::atomic<uint64_t> g_launches{0};
+bool g_profile = false;
+std::vector<ProfRec> g_prof;
+void prof_push(int kind, cudaEvent_t a, cudaEvent_t b) { g_prof.push_back({kind, a, b}); }
 }
-
-#define VC_LAUNCH(kern, grid, block, smem, stream, ...)                     \
-    do {                                                                    \
-        kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);           \
-        vc::g_launches.fetch_add(1, std::memory_order_relaxed);            \
-    } while (0)
 
 #define CUDA_TRY(x)                                          \
     do {                                                     \
@@ -58,6 +55,7 @@ extern "C" const char *vc_strerror(int code) {
 
 extern "C" void vc_circuit_free(vc_circuit *c) {
     if (!c) return;
+    vc::fused_free(c);
     for (auto p : c->d_type) cudaFree(p);
     for (auto p : c->d_in1) cudaFree(p);
     for (auto p : c->d_in2) cudaFree(p);
@@ -159,10 +157,10 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const uint32_t d = c->d;
     const uint64_t n_in = 1ull << c->log_input;
-    VC_LAUNCH(vc::k_copy_input, grid_for(n_in, c->sm_count), vc::RED_BLOCK, 0, st, d_input, c->d_V[d], n_in, c->d_state);
+    VC_LAUNCH(VC_K_EVAL, vc::k_copy_input, grid_for(n_in, c->sm_count), vc::RED_BLOCK, 0, st, d_input, c->d_V[d], n_in, c->d_state);
     for (int i = (int)d - 1; i >= 0; i--) {
         const uint32_t n = 1u << c->logs[i];
-        VC_LAUNCH(vc::k_eval, grid_for(n, c->sm_count, 2), vc::RED_BLOCK, 0, st, c->d_type[i], c->d_in1[i], c->d_in2[i],
+        VC_LAUNCH(VC_K_EVAL, vc::k_eval, grid_for(n, c->sm_count, 2), vc::RED_BLOCK, 0, st, c->d_type[i], c->d_in1[i], c->d_in2[i],
                   c->d_V[i + 1], c->d_V[i], (i == 0 ? d_outputs : (uint64_t *)nullptr), n);
     }
     CUDA_TRY(cudaGetLastError());
@@ -180,9 +178,9 @@ int vc::enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, ui
     const uint64_t *Vb = c->d_V[layer + 1];
     const uint32_t gg = grid_for(n, c->sm_count);
     const uint32_t cb = si < (uint32_t)vc::BETA_LOG_CHUNK ? si : (uint32_t)vc::BETA_LOG_CHUNK;
-    if (layer == 0) VC_LAUNCH(vc::k_start, 1, 64, 0, st, S, seed, si);
-    VC_LAUNCH(vc::k_beta, 1u << (si - cb), 256, 0, st, S, c->d_P, si);
-    if (layer == 0) VC_LAUNCH(vc::k_dot_claim, gg, vc::RED_BLOCK, 0, st, c->d_P, c->d_V[0], n, c->d_part, S);
+    if (layer == 0) VC_LAUNCH(VC_K_SETUP, vc::k_start, 1, 64, 0, st, S, seed, si);
+    VC_LAUNCH(VC_K_SETUP, vc::k_beta, 1u << (si - cb), 256, 0, st, S, c->d_P, si);
+    if (layer == 0) VC_LAUNCH(VC_K_SETUP, vc::k_dot_claim, gg, vc::RED_BLOCK, 0, st, c->d_P, c->d_V[0], n, c->d_part, S);
     uint64_t *tr = d_tr;
     for (int phase = 1; phase <= 2; phase++) {
         const uint64_t *tab = Vb;
@@ -191,18 +189,18 @@ int vc::enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, ui
             const uint32_t half = 1u << (s - j - 1);
             const uint32_t gu = grid_for(std::max(n, half), c->sm_count);
             if (phase == 1) {
-                VC_LAUNCH(vc::k_round<1>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
-                VC_LAUNCH(vc::k_update<1>, gu, vc::RED_BLOCK, 0, st, in1, c->d_P, tab, out, S, j, n, half);
+                VC_LAUNCH(VC_K_ROUND, vc::k_round<1>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
+                VC_LAUNCH(VC_K_UPDATE, vc::k_update<1>, gu, vc::RED_BLOCK, 0, st, in1, c->d_P, tab, out, S, j, n, half);
             } else {
-                VC_LAUNCH(vc::k_round<2>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
-                VC_LAUNCH(vc::k_update<2>, gu, vc::RED_BLOCK, 0, st, in2, c->d_P, tab, out, S, j, n, half);
+                VC_LAUNCH(VC_K_ROUND, vc::k_round<2>, gg, vc::RED_BLOCK, 0, st, type, in1, in2, c->d_P, tab, Vb, S, j, n, c->d_part, tr);
+                VC_LAUNCH(VC_K_UPDATE, vc::k_update<2>, gu, vc::RED_BLOCK, 0, st, in2, c->d_P, tab, out, S, j, n, half);
             }
             tab = out;
             tr += 3;
         }
     }
     const uint32_t used = std::min<uint32_t>(s, vc::LINE_NT + vc::LINE_TB);
-    VC_LAUNCH(vc::k_line, 1u << (s - used), 256, vc::line_smem_words(s) * 8, st, Vb, s, S, c->d_part, tr);
+    VC_LAUNCH(VC_K_LINE, vc::k_line, 1u << (s - used), 256, vc::line_smem_words(s) * 8, st, Vb, s, S, c->d_part, tr);
     return cudaGetLastError() == cudaSuccess ? VC_OK : VC_ERR_CUDA;
 }
 
@@ -227,6 +225,13 @@ extern "C" int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, ui
     if (!c || !d_transcript) return VC_ERR_ARG;
     if (cap_words < c->total_words) return VC_ERR_ARG;
     if (c->next_layer != 0) return VC_ERR_STATE;
+    if (c->schedule != 1 && vc::fused_supported(c, 0)) {     // whole proof in one cooperative launch
+        int rc = vc::enqueue_layers_fused(c, 0, c->d, seed, d_transcript, (cudaStream_t)cuda_stream);
+        if (rc != VC_OK) return rc;
+        c->seed = seed;
+        c->next_layer = (int)c->d;
+        return VC_OK;
+    }
     uint64_t w = 0;
     for (uint32_t i = 0; i < c->d; i++) {
         const uint64_t nw = 7ull * c->logs[i + 1] + 1;
@@ -331,7 +336,7 @@ extern "C" int vc_debug_fieldop(int op, const uint64_t *d_a, const uint64_t *d_b
                                 void *cuda_stream) {
     if (!d_a || !d_b || !d_out || op < 0 || op > 4) return VC_ERR_ARG;
     if (n == 0) return VC_OK;
-    VC_LAUNCH(vc::k_fieldop, (uint32_t)std::min<uint64_t>((n + 255) / 256, 1184), 256, 0, (cudaStream_t)cuda_stream, op, d_a, d_b, d_out, n);
+    VC_LAUNCH(VC_K_MISC, vc::k_fieldop, (uint32_t)std::min<uint64_t>((n + 255) / 256, 1184), 256, 0, (cudaStream_t)cuda_stream, op, d_a, d_b, d_out, n);
     CUDA_TRY(cudaGetLastError());
     return VC_OK;
 }
@@ -340,12 +345,33 @@ extern "C" int vc_bench_modmul(uint32_t grid, uint32_t block, uint32_t iters, ui
     if (!d_out || grid == 0 || block == 0 || block > 1024) return VC_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     switch (ilp) {
-    case 1: VC_LAUNCH(vc::k_bench_modmul<1>, grid, block, 0, st, iters, d_out); break;
-    case 2: VC_LAUNCH(vc::k_bench_modmul<2>, grid, block, 0, st, iters, d_out); break;
-    case 4: VC_LAUNCH(vc::k_bench_modmul<4>, grid, block, 0, st, iters, d_out); break;
-    case 8: VC_LAUNCH(vc::k_bench_modmul<8>, grid, block, 0, st, iters, d_out); break;
+    case 1: VC_LAUNCH(VC_K_MISC, vc::k_bench_modmul<1>, grid, block, 0, st, iters, d_out); break;
+    case 2: VC_LAUNCH(VC_K_MISC, vc::k_bench_modmul<2>, grid, block, 0, st, iters, d_out); break;
+    case 4: VC_LAUNCH(VC_K_MISC, vc::k_bench_modmul<4>, grid, block, 0, st, iters, d_out); break;
+    case 8: VC_LAUNCH(VC_K_MISC, vc::k_bench_modmul<8>, grid, block, 0, st, iters, d_out); break;
     default: return VC_ERR_ARG;
     }
     CUDA_TRY(cudaGetLastError());
+    return VC_OK;
+}
+
+// ------------------------------------------------------------------ per-kernel-kind timing for bench.py's roofline
+extern "C" int vc_profile_enable(int on) {
+    for (auto &r : vc::g_prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    vc::g_prof.clear();
+    vc::g_profile = on != 0;
+    return VC_OK;
+}
+extern "C" int vc_profile_read(uint64_t *launches, double *ms) {
+    if (!launches || !ms) return VC_ERR_ARG;
+    CUDA_TRY(cudaDeviceSynchronize());
+    for (int k = 0; k < VC_K_COUNT; k++) { launches[k] = 0; ms[k] = 0.0; }
+    for (auto &r : vc::g_prof) {
+        float t = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&t, r.a, r.b));
+        launches[r.kind] += 1; ms[r.kind] += t;
+        cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+    }
+    vc::g_prof.clear();
     return VC_OK;
 }

@@ -42,8 +42,23 @@ struct vc_circuit {
 
 namespace vc {
 extern std::atomic<uint64_t> g_launches;
+struct ProfRec { int kind; cudaEvent_t a, b; };
+extern bool g_profile;                      // vc_profile_enable: CUDA events around every launch, by kind
+void prof_push(int kind, cudaEvent_t a, cudaEvent_t b);
 int enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
 int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);  // vc_fused.cu
 int fused_supported(const vc_circuit *c, uint32_t layer);
 int fused_init(vc_circuit *c);
+void fused_free(const vc_circuit *c);
+int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
 }  // namespace vc
+
+// Launch + count (+ optional event pair tagged with the kernel kind, for bench.py's live roofline numbers).
+#define VC_LAUNCH(kind, kern, grid, block, smem, stream, ...)                               \
+    do {                                                                                    \
+        cudaEvent_t ea_ = nullptr, eb_ = nullptr;                                           \
+        if (vc::g_profile) { cudaEventCreate(&ea_); cudaEventCreate(&eb_); cudaEventRecord(ea_, (stream)); } \
+        kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                           \
+        if (vc::g_profile) { cudaEventRecord(eb_, (stream)); vc::prof_push((kind), ea_, eb_); } \
+        vc::g_launches.fetch_add(1, std::memory_order_relaxed);                             \
+    } while (0)

@@ -77,7 +77,7 @@ __device__ __forceinline__ bool grid_sum_last_block(uint64_t (&v)[K], uint64_t *
 
 // ------------------------------------------------------------------ a1: evaluation
 // V_d <- input (checked canonical)
-__global__ void k_copy_input(const uint64_t *in, uint64_t *out, uint64_t n, DevState *st) {  // in may equal out
+static __global__ void k_copy_input(const uint64_t *in, uint64_t *out, uint64_t n, DevState *st) {  // in may equal out
     unsigned bad = 0;
     for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         uint64_t w = in[i];
@@ -97,7 +97,7 @@ __device__ __forceinline__ uint64_t gate_f(uint32_t t, uint64_t L, uint64_t R) {
 }
 
 // V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]])   (all gates of a layer in parallel)
-__global__ void k_eval(const uint8_t *__restrict__ type, const uint32_t *__restrict__ in1,
+static __global__ void k_eval(const uint8_t *__restrict__ type, const uint32_t *__restrict__ in1,
                        const uint32_t *__restrict__ in2, const uint64_t *__restrict__ Vb,
                        uint64_t *__restrict__ Vout, uint64_t *__restrict__ Vout2, uint32_t n) {
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
@@ -109,7 +109,7 @@ __global__ void k_eval(const uint8_t *__restrict__ type, const uint32_t *__restr
 
 // ------------------------------------------------------------------ a2: start of the proof
 // ctr <- 0; z_0 <- s0 draws.  One warp-sized block.
-__global__ void k_start(DevState *st, uint64_t seed, uint32_t s0) {
+static __global__ void k_start(DevState *st, uint64_t seed, uint32_t s0) {
     for (uint32_t k = threadIdx.x; k < s0; k += blockDim.x) st->z[k] = fp61::draw(seed, k);
     if (threadIdx.x == 0) { st->seed = seed; st->ctr = s0; st->ticket = 0; }
 }
@@ -119,7 +119,7 @@ __global__ void k_start(DevState *st, uint64_t seed, uint32_t s0) {
 // T[u + 2^k] = T[u] z_k ; T[u] -= T[u + 2^k]   (1 multiply per new entry), seeded with the product
 // over the bits >= c that are fixed for the chunk.
 constexpr int BETA_LOG_CHUNK = 11;
-__global__ void __launch_bounds__(256) k_beta(const DevState *__restrict__ st, uint64_t *__restrict__ Pw, uint32_t s) {
+static __global__ void __launch_bounds__(256) k_beta(const DevState *__restrict__ st, uint64_t *__restrict__ Pw, uint32_t s) {
     __shared__ uint64_t T[1 << BETA_LOG_CHUNK];
     const uint32_t c = s < BETA_LOG_CHUNK ? s : BETA_LOG_CHUNK;
     const uint32_t base = blockIdx.x << c;
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(256) k_beta(const DevState *__restrict__ st, u
 }
 
 // claim <- sum_g P[g] V_0[g] = V~_0(z_0)
-__global__ void __launch_bounds__(RED_BLOCK) k_dot_claim(const uint64_t *__restrict__ Pw, const uint64_t *__restrict__ V,
+static __global__ void __launch_bounds__(RED_BLOCK) k_dot_claim(const uint64_t *__restrict__ Pw, const uint64_t *__restrict__ V,
                                                           uint32_t n, uint64_t *part, DevState *st) {
     __shared__ uint64_t red[32];
     acc128 a; a.clear();

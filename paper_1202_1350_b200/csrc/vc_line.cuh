@@ -19,7 +19,7 @@ __host__ __device__ inline size_t line_smem_words(uint32_t s) {
     return m * s + m * 256 + m * 8 + (s + 1) + 32;
 }
 
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 k_line(const uint64_t *__restrict__ Vb, uint32_t s, DevState *st, uint64_t *part, uint64_t *tr_q) {
     extern __shared__ uint64_t sm[];
     __shared__ int s_last;
