@@ -97,6 +97,8 @@ uint32_t vc_log_size(const vc_circuit *c, uint32_t layer);           /* layer = 
 int vc_debug_state(const vc_circuit *c, uint64_t *h_z64, uint64_t *h_claim, uint64_t *h_ctr, void *cuda_stream);
 /* copies value table V_layer (layer = d: the input copy) to the host */
 int vc_debug_values(const vc_circuit *c, uint32_t layer, uint64_t *h_values, void *cuda_stream);
+/* fused schedule only: d+1 device timestamps (ns, %globaltimer): start of each layer's proof, [d] = end */
+int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *cuda_stream);
 /* sticky device-side status: 0 = fine, 1 = a non-canonical input word was seen by vc_evaluate */
 int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */

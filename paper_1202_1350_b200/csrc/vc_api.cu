@@ -294,6 +294,11 @@ extern "C" int vc_debug_values(const vc_circuit *c, uint32_t layer, uint64_t *h_
     return VC_OK;
 }
 
+extern "C" int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *cuda_stream) {
+    if (!c || !h_ns) return VC_ERR_ARG;
+    return vc::fused_stamps(c, h_ns, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream) {
     if (!c || !h_flags) return VC_ERR_ARG;
     CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));

@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     bool handoff = false;                         // CTA 0 ran narrow layers alone: publish its state first
     for (uint32_t layer = a.begin; layer < a.end; layer++) {
         const uint32_t s = a.L[layer + 1].log_n;
+        if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
         if (is_small(a, layer)) {
             if (blockIdx.x == 0) small_layer(a, cx, dyn, layer, tr);
             handoff = true;
@@ -56,6 +57,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         tr += 7 * (size_t)s + 1;
     }
     // ---- leave the state for the next call
+    if (blockIdx.x == 0 && tid == 0) a.stamps[a.end] = globaltimer_ns();
     if (blockIdx.x == 0) {
         if (tid < MAX_VARS) a.st->z[tid] = cx.z[tid];
         if (tid == 0) { a.st->seed = cx.seed; a.st->ctr = cx.ctr; a.st->claim = cx.claim; a.st->bar_gen = cx.epoch; }
@@ -65,6 +67,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
 struct FusedHost {
     LayerDesc *d_desc = nullptr;
     unsigned long long *d_slots = nullptr;
+    uint64_t *d_stamps = nullptr;
     int grid = 0;
 };
 static std::vector<std::pair<const vc_circuit *, FusedHost>> g_fused;
@@ -98,6 +101,8 @@ int fused_init(vc_circuit *c) {
     }
     if (cudaMalloc(&fh.d_desc, h.size() * sizeof(LayerDesc)) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_slots, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_desc, h.data(), h.size() * sizeof(LayerDesc), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemset(fh.d_slots, 0, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_CUDA;
     g_fused.emplace_back(c, fh);
@@ -109,6 +114,7 @@ void fused_free(const vc_circuit *c) {
         if (g_fused[i].first == c) {
             cudaFree(g_fused[i].second.d_desc);
             cudaFree(g_fused[i].second.d_slots);
+            cudaFree(g_fused[i].second.d_stamps);
             g_fused.erase(g_fused.begin() + i);
             return;
         }
@@ -122,7 +128,7 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
     if (!fh) return VC_ERR_STATE;
     FusedArgs a;
     a.L = fh->d_desc; a.d = c->d; a.begin = begin; a.end = end; a.seed = seed; a.st = c->d_state; a.tr = d_tr;
-    a.P = c->d_P; a.T0 = c->d_T0; a.T1 = c->d_T1; a.slots = fh->d_slots;
+    a.P = c->d_P; a.T0 = c->d_T0; a.T1 = c->d_T1; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
     void *params[] = {&a};
     cudaEvent_t ea = nullptr, eb = nullptr;
     if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
@@ -131,6 +137,13 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
     return VC_OK;
+}
+
+int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st) {
+    FusedHost *fh = find(c);
+    if (!fh) return VC_ERR_STATE;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return VC_ERR_CUDA;
+    return cudaMemcpy(h, fh->d_stamps, (size_t)(c->d + 1) * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? VC_OK : VC_ERR_CUDA;
 }
 
 int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {

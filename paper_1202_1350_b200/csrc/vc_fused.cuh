@@ -41,6 +41,7 @@ struct FusedArgs {
     uint64_t *tr;            // transcript position of layer `begin`
     uint64_t *P, *T0, *T1;   // global scratch (streaming-mode weights; fold tables)
     unsigned long long *slots;  // F_RING * F_SLOT_WORDS words, all zero between launches
+    uint64_t *stamps;        // d+1 words: %globaltimer (ns) when CTA 0 starts layer i, [d] = end of the proof
 };
 
 struct FusedCtx {            // block-shared bookkeeping, replicated in every CTA
@@ -62,6 +63,11 @@ __device__ __forceinline__ unsigned long long ld_acquire(const unsigned long lon
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
 }
 __device__ __forceinline__ void red_add(unsigned long long *p, unsigned long long v) {
     asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
