@@ -1,4 +1,4 @@
-// vc_fused.cu — kernel + host driver of the on-chip schedule (see vc_fused.cuh).
+// vc_fused.cu — kernel + host driver (load-time plan, launch) of the on-chip schedule (see vc_fused.cuh).
 #include <algorithm>
 #include <vector>
 
@@ -8,14 +8,11 @@
 
 namespace vc {
 
-__device__ __forceinline__ bool is_small(const FusedArgs &a, uint32_t layer) {
-    return a.L[layer].log_n <= F_SMALL_N_LOG && a.L[layer + 1].log_n <= F_SMALL_T_LOG;
-}
-
 __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     extern __shared__ __align__(16) uint8_t smem[];
     FusedCtx &cx = *reinterpret_cast<FusedCtx *>(smem);
-    uint8_t *dyn = smem + sizeof(FusedCtx);
+    uint64_t *invfact = reinterpret_cast<uint64_t *>(smem + sizeof(FusedCtx));      // 1/k!, k <= MAX_VARS
+    uint8_t *dyn = smem + F_FIXED_BYTES;
     const uint32_t tid = threadIdx.x;
     // ---- load (or start) the proof state
     if (a.begin == 0) {
@@ -26,6 +23,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (tid < MAX_VARS) cx.z[tid] = a.st->z[tid];
         if (tid == 0) { cx.seed = a.seed; cx.ctr = a.st->ctr; cx.claim = a.st->claim; }
     }
+    if (tid <= MAX_VARS) invfact[tid] = a.st->invfact[tid];
     if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; }
     __syncthreads();
     uint64_t *tr = a.tr;
@@ -33,8 +31,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     for (uint32_t layer = a.begin; layer < a.end; layer++) {
         const uint32_t s = a.L[layer + 1].log_n;
         if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
-        if (is_small(a, layer)) {
-            if (blockIdx.x == 0) small_layer(a, cx, dyn, layer, tr);
+        if (a.L[layer].kind == 0) {
+            if (blockIdx.x == 0) small_layer(a, cx, invfact, dyn, layer, tr);
             handoff = true;
         } else {
             if (handoff) {
@@ -42,7 +40,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                     if (tid < MAX_VARS) a.st->z[tid] = cx.z[tid];
                     if (tid == 0) { a.st->ctr = cx.ctr; a.st->claim = cx.claim; }
                 }
-                grid_allreduce(cx, a, 0);
+                grid_allreduce(cx, a, 0, true);
                 if (blockIdx.x != 0) {
                     if (tid < MAX_VARS) cx.z[tid] = __ldcg(&a.st->z[tid]);
                     if (tid == 0) { cx.ctr = __ldcg(&a.st->ctr); cx.claim = __ldcg(&a.st->claim); }
@@ -50,9 +48,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                 __syncthreads();
                 handoff = false;
             }
-            const uint32_t nch0 = (1u << a.L[layer].log_n) >> F_CHUNK_LOG, nch = nch0 ? nch0 : 1u;
-            if ((nch + gridDim.x - 1) / gridDim.x <= (uint32_t)F_MAXK) wide_layer<true>(a, cx, dyn, layer, tr);
-            else wide_layer<false>(a, cx, dyn, layer, tr);
+            if (a.L[layer].resident) wide_layer<true>(a, cx, invfact, dyn, layer, tr);
+            else wide_layer<false>(a, cx, invfact, dyn, layer, tr);
         }
         tr += 7 * (size_t)s + 1;
     }
@@ -64,11 +61,15 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     }
 }
 
+constexpr size_t F_SMEM_MAX = 227 * 1024;
+
 struct FusedHost {
-    LayerDesc *d_desc = nullptr;
+    LayerPlan *d_plan = nullptr;
+    CtaPlan *d_cta = nullptr;
     unsigned long long *d_slots = nullptr;
-    uint64_t *d_stamps = nullptr;
+    uint64_t *d_stamps = nullptr, *d_C = nullptr, *d_Tg = nullptr;
     int grid = 0;
+    size_t smem = 0;
 };
 static std::vector<std::pair<const vc_circuit *, FusedHost>> g_fused;
 
@@ -77,33 +78,120 @@ static FusedHost *find(const vc_circuit *c) {
     return nullptr;
 }
 
+// ---- the load-time plan: how each layer is partitioned over the CTAs, which table mode each phase uses and where
+// its buffers sit in shared memory.  Pure index bookkeeping on the host copy of the records.
+static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, std::vector<CtaPlan> &cta, size_t &smem_need) {
+    const uint32_t si = c->logs[i], s = c->logs[i + 1];
+    const uint64_t n = 1ull << si;
+    lp.log_n = si;
+    lp.kind = (si <= (uint32_t)F_SMALL_N_LOG && s <= (uint32_t)F_SMALL_T_LOG) ? 0 : 1;
+    lp.resident = 0; lp.cap = 0; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
+    lp.xw = lp.yw = 0; lp.off_tab = lp.off_scr = 0;
+    if (lp.kind == 0) { smem_need = std::max(smem_need, F_FIXED_BYTES + F_SMALL_BYTES); return; }
+    // gates in units of 32, spread evenly over the CTAs
+    const uint64_t U = (n + 31) / 32;
+    uint64_t ngmax = 0;
+    cta.assign(G, CtaPlan{});
+    const uint32_t K = s > (uint32_t)F_TLOG ? s - F_TLOG : 0;
+    uint64_t nbmax[2] = {0, 0};
+    for (int b = 0; b < G; b++) {
+        const uint64_t g0 = std::min<uint64_t>(n, 32 * ((uint64_t)b * U / G)), g1 = std::min<uint64_t>(n, 32 * ((uint64_t)(b + 1) * U / G));
+        cta[b].g0 = (uint32_t)g0; cta[b].g1 = (uint32_t)g1;
+        ngmax = std::max(ngmax, g1 - g0);
+        for (int ph = 0; ph < 2; ph++) {
+            const std::vector<uint32_t> &idx = ph == 0 ? c->h_in1[i] : c->h_in2[i];
+            uint32_t lo = 0xffffffffu, hi = 0;
+            for (uint64_t g = g0; g < g1; g++) { lo = std::min(lo, idx[g]); hi = std::max(hi, idx[g]); }
+            if (g1 > g0) { cta[b].blo[ph] = lo >> K; cta[b].nb[ph] = (hi >> K) - (lo >> K) + 1; }
+            nbmax[ph] = std::max<uint64_t>(nbmax[ph], cta[b].nb[ph]);
+        }
+    }
+    const size_t cap = (size_t)((ngmax + FT - 1) / FT) * FT;
+    const size_t state = cap * 20;
+    // fold buffers: odd levels in X, even levels in Y; slices exist for levels 1..K-1
+    auto buf_words = [&](int ph, size_t &xw, size_t &yw) {
+        xw = (size_t)1 << (s >= 1 ? std::min<uint32_t>(s - 1, F_TLOG) : 0);
+        yw = (size_t)1 << (s >= 2 ? std::min<uint32_t>(s - 2, F_TLOG) : 0);
+        if (K >= 2) xw = std::max(xw, (size_t)nbmax[ph] << (K - 1));
+        if (K >= 3) yw = std::max(yw, (size_t)nbmax[ph] << (K - 2));
+    };
+    const size_t scr_words = 1u << F_EQLOG;
+    bool slice_ok[2];
+    for (int ph = 0; ph < 2; ph++) slice_ok[ph] = K <= (uint32_t)F_EQLOG + 1;   // the owner's eq table covers K-1 <= 10 variables
+    // try: resident state + slices, then non-resident + slices, then drop the larger slice, ...
+    for (int attempt = 0; attempt < 6; attempt++) {
+        const bool res = attempt < 3;
+        const int drop = attempt % 3;            // 0: both phases sliced, 1: drop the larger, 2: drop both
+        bool use[2] = {slice_ok[0], slice_ok[1]};
+        size_t xw[2], yw[2];
+        buf_words(0, xw[0], yw[0]); buf_words(1, xw[1], yw[1]);
+        if (drop >= 1) { const int big = (xw[0] + yw[0] >= xw[1] + yw[1]) ? 0 : 1; use[big] = false; }
+        if (drop >= 2) use[0] = use[1] = false;
+        size_t X = 1024, Y = 1024;
+        for (int ph = 0; ph < 2; ph++) if (use[ph]) { X = std::max(X, xw[ph]); Y = std::max(Y, yw[ph]); }
+        X = (X + 1) & ~(size_t)1; Y = (Y + 1) & ~(size_t)1;
+        const size_t tabw = std::max<size_t>(X + Y, std::max<size_t>(4u << F_EQLOG, fused_line_words(s)));
+        const size_t st_bytes = res ? state : 0;
+        const size_t total = F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8;
+        if (total > F_SMEM_MAX) continue;
+        if (res && cap > 8u * FT) continue;      // accumulators hold 8 products between reductions either way; keep the resident loop short
+        lp.resident = res ? 1 : 0;
+        lp.cap = (uint32_t)cap;
+        for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = use[ph] ? F_MODE_SLICE : F_MODE_GLOBAL; lp.K[ph] = K; }
+        lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
+        lp.off_tab = (uint32_t)st_bytes;
+        lp.off_scr = (uint32_t)(st_bytes + tabw * 8);
+        smem_need = std::max(smem_need, total);
+        return;
+    }
+    // unreachable: the last attempt (non-resident, no slices) needs only the fixed buffers
+}
+
 int fused_init(vc_circuit *c) {
     if (!c->coop_ok) return VC_OK;
     FusedHost fh;
-    if (cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_BYTES) != cudaSuccess) {
+    fh.grid = c->sm_count;
+    std::vector<LayerPlan> h(c->d + 1);
+    std::vector<CtaPlan> all_cta;
+    std::vector<size_t> cta_off(c->d + 1, (size_t)-1);
+    size_t smem_need = F_FIXED_BYTES + F_SMALL_BYTES;
+    for (uint32_t i = 0; i <= c->d; i++) {
+        LayerPlan &lp = h[i];
+        lp = LayerPlan{};
+        lp.type = i < c->d ? c->d_type[i] : nullptr;
+        lp.in1 = i < c->d ? c->d_in1[i] : nullptr;
+        lp.in2 = i < c->d ? c->d_in2[i] : nullptr;
+        lp.V = c->d_V[i];
+        lp.log_n = c->logs[i];
+        if (i < c->d) {
+            std::vector<CtaPlan> cta;
+            plan_layer(c, i, fh.grid, lp, cta, smem_need);
+            if (lp.kind == 1) { cta_off[i] = all_cta.size(); all_cta.insert(all_cta.end(), cta.begin(), cta.end()); }
+        }
+    }
+    fh.smem = smem_need;
+    if (cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess) {
         (void)cudaGetLastError();
         return VC_OK;                                // no fused schedule on this device; streaming still works
     }
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fused, FT, F_SMEM_BYTES) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fused, FT, fh.smem) != cudaSuccess || per_sm < 1) {
         (void)cudaGetLastError();
         return VC_OK;
     }
-    fh.grid = c->sm_count;
-    std::vector<LayerDesc> h(c->d + 1);
-    for (uint32_t i = 0; i <= c->d; i++) {
-        h[i].type = i < c->d ? c->d_type[i] : nullptr;
-        h[i].in1 = i < c->d ? c->d_in1[i] : nullptr;
-        h[i].in2 = i < c->d ? c->d_in2[i] : nullptr;
-        h[i].V = c->d_V[i];
-        h[i].log_n = c->logs[i];
-        h[i].pad = 0;
-    }
-    if (cudaMalloc(&fh.d_desc, h.size() * sizeof(LayerDesc)) != cudaSuccess) return VC_ERR_NOMEM;
+    uint64_t max_gates = 1;
+    for (uint32_t i = 0; i < c->d; i++) max_gates = std::max<uint64_t>(max_gates, 1ull << c->logs[i]);
+    if (cudaMalloc(&fh.d_plan, h.size() * sizeof(LayerPlan)) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_cta, std::max<size_t>(all_cta.size(), 1) * sizeof(CtaPlan)) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_slots, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_C, max_gates * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_Tg, (size_t)(2u << F_TLOG) * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_CUDA;
-    if (cudaMemcpy(fh.d_desc, h.data(), h.size() * sizeof(LayerDesc), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
+    if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
+    if (!all_cta.empty() &&
+        cudaMemcpy(fh.d_cta, all_cta.data(), all_cta.size() * sizeof(CtaPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemset(fh.d_slots, 0, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_CUDA;
     g_fused.emplace_back(c, fh);
     return VC_OK;
@@ -112,9 +200,8 @@ int fused_init(vc_circuit *c) {
 void fused_free(const vc_circuit *c) {
     for (size_t i = 0; i < g_fused.size(); i++)
         if (g_fused[i].first == c) {
-            cudaFree(g_fused[i].second.d_desc);
-            cudaFree(g_fused[i].second.d_slots);
-            cudaFree(g_fused[i].second.d_stamps);
+            FusedHost &f = g_fused[i].second;
+            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg);
             g_fused.erase(g_fused.begin() + i);
             return;
         }
@@ -127,12 +214,12 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
     FusedHost *fh = find(c);
     if (!fh) return VC_ERR_STATE;
     FusedArgs a;
-    a.L = fh->d_desc; a.d = c->d; a.begin = begin; a.end = end; a.seed = seed; a.st = c->d_state; a.tr = d_tr;
-    a.P = c->d_P; a.T0 = c->d_T0; a.T1 = c->d_T1; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
+    a.L = fh->d_plan; a.d = c->d; a.begin = begin; a.end = end; a.seed = seed; a.st = c->d_state; a.tr = d_tr;
+    a.P = c->d_P; a.C = fh->d_C; a.T0 = c->d_T0; a.T1 = c->d_T1; a.Tg = fh->d_Tg; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
     void *params[] = {&a};
     cudaEvent_t ea = nullptr, eb = nullptr;
     if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
-    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_fused, dim3(fh->grid), dim3(FT), params, F_SMEM_BYTES, st);
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_fused, dim3(fh->grid), dim3(FT), params, fh->smem, st);
     if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_FUSED_WIDE, ea, eb); }
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }

@@ -1,45 +1,65 @@
-// vc_fused.cuh — the on-chip ("fused") schedule: ONE persistent cooperative kernel walks a range of layers;
-// the per-gate state (weight P, fixed operand, packed record) of a layer stays in shared memory across all of
-// its rounds, the three round values are all-reduced through one 64-byte L2 line per round, and every CTA draws
-// the challenge itself, so a round costs one grid-wide rendezvous and no kernel launch.
+// vc_fused.cuh — the on-chip ("fused") schedule: ONE persistent cooperative kernel walks all layers of the proof.
 //
-// Same method as the streaming schedule (every gate contributes independently to every
-// message); what changes is where the data lives and how the chain of dependent rounds
-// is synchronised (SURVEY.md §7 "Round latency, not bandwidth, is the first wall").
-//
-// Layers with at most 2^10 gates and a table of at most 2^12 words are proved by CTA 0 alone out of shared
-// memory (block barriers only) while the other CTAs wait at the next grid rendezvous.
+// Same method as the streaming schedule (every gate contributes independently to every message,
+// contributions are reduced in F_p).  What changes is where the data lives and how the chain
+// of strictly dependent rounds is synchronised (SURVEY.md §7 "Round latency, not bandwidth, is the first wall"):
+//   * per-gate state (W, c, idx) stays in shared memory across all 2s rounds of a layer (the paper's "no-copying
+//     approach", pushed one level further up the memory hierarchy);
+//   * every gate's contribution is W * (x + c): for MULT the fixed operand is folded into the weight once per phase
+//     (W = P * V[in2]), for ADD/SUB/RELAY it is the additive constant c, so the hot loop has no per-type branch and
+//     costs 3 wide multiplies per gate-round;
+//   * fold tables live in shared memory: each CTA folds the slice its gates read (levels < K) and, from level K on,
+//     the whole (<= 2^10-entry) table, redundantly; level K-1 is published through L2 once per phase;
+//   * the three round values are all-reduced through one L2 line per round (red.add + polling), after which every
+//     CTA draws the challenge itself: one grid rendezvous per round, no kernel launch, no host round-trip.
+// Challenges are only ever used AFTER the message they answer has been completely reduced (causality of the
+// interactive protocol), although the seeded generator would allow drawing them earlier.
 #pragma once
 #include "vc_kernels.cuh"
-#include "vc_line.cuh"
-#include "vc_round.cuh"
 
 namespace vc {
 
 constexpr int FT = 1024;                 // threads per CTA
-constexpr int F_CHUNK_LOG = 10;          // a chunk = 1024 consecutive gates = one gate per thread
-constexpr int F_MAXK = 8;                // chunks per CTA that fit in shared memory
+constexpr int F_TLOG = 10;               // the fully shared part of a fold table has 2^min(s, F_TLOG) entries
+constexpr int F_EQLOG = 10;              // eq tables are built in halves of at most 2^10 entries
 constexpr int F_SMALL_N_LOG = 10;        // single-CTA path: gates <= 2^10 ...
 constexpr int F_SMALL_T_LOG = 12;        // ... and table <= 2^12 words
 constexpr int F_SLOT_WORDS = 128;        // one rendezvous slot: up to 64 values x (lo,hi)
 constexpr int F_RING = 4;
 constexpr uint64_t F_CNT_ONE = 1ull << 48;
 constexpr uint64_t F_VAL_MASK = F_CNT_ONE - 1;
+constexpr uint32_t F_IDX_MASK = 0x3fffffffu;   // indices are < 2^30; bit 31 of a packed index = "x ignored" (RELAY, phase 2)
+constexpr int F_MODE_SLICE = 0, F_MODE_GLOBAL = 1;
 
-struct LayerDesc {
+struct CtaPlan {                         // per (wide layer, CTA), computed at load from the host copy of the records
+    uint32_t g0, g1;                     // gates [g0, g1) of the layer
+    uint32_t blo[2], nb[2];              // per phase: first level-K block its gates read, and how many
+};
+
+struct LayerPlan {
     const uint8_t *type;
     const uint32_t *in1, *in2;
-    const uint64_t *V;       // values of this layer (entry d: the input)
-    uint32_t log_n, pad;
+    const uint64_t *V;                   // values of this layer (entry d: the input)
+    const CtaPlan *cta;                  // gridDim entries (wide layers), else null
+    uint32_t log_n;
+    uint32_t kind;                       // 0: single CTA, 1: grid-wide
+    uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
+    uint32_t cap;                        // state capacity in gates (multiple of FT)
+    uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
+    uint32_t K[2];                       // per phase: first fully shared level
+    uint32_t xw, yw;                     // words of the two fold buffers
+    uint32_t off_tab, off_scr;           // byte offsets in dynamic shared memory (after the state)
 };
 
 struct FusedArgs {
-    const LayerDesc *L;      // d+1 descriptors
+    const LayerPlan *L;      // d+1 descriptors
     uint32_t d, begin, end;  // prove layers [begin, end)
     uint64_t seed;
     DevState *st;
     uint64_t *tr;            // transcript position of layer `begin`
-    uint64_t *P, *T0, *T1;   // global scratch (streaming-mode weights; fold tables)
+    uint64_t *P, *C;         // global scratch: non-resident gate state (W, c)
+    uint64_t *T0, *T1;       // global fold tables (F_MODE_GLOBAL)
+    uint64_t *Tg;            // published level K-1 (F_MODE_SLICE), 2^(F_TLOG+1) words
     unsigned long long *slots;  // F_RING * F_SLOT_WORDS words, all zero between launches
     uint64_t *stamps;        // d+1 words: %globaltimer (ns) when CTA 0 starts layer i, [d] = end of the proof
 };
@@ -47,14 +67,14 @@ struct FusedArgs {
 struct FusedCtx {            // block-shared bookkeeping, replicated in every CTA
     uint64_t z[MAX_VARS], r1[MAX_VARS], r2[MAX_VARS], q[MAX_VARS + 1];
     uint64_t acc[MAX_VARS];
-    uint64_t red[3 * 32];
+    uint64_t red[32 * 4];    // per-warp partials of a round
     uint64_t G[4];
     uint64_t seed, ctr, claim, v1, v2;
     uint32_t epoch, pad;
 };
 
-constexpr size_t F_STATE_BYTES = (size_t)F_MAXK * FT * (8 + 8 + 4 + 4);
-constexpr size_t F_SMEM_BYTES = sizeof(FusedCtx) + F_STATE_BYTES;
+// fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS; the rest starts 16-byte aligned
+constexpr size_t F_FIXED_BYTES = (sizeof(FusedCtx) + (MAX_VARS + 1) * 8 + 15) & ~(size_t)15;
 
 __device__ __forceinline__ uint64_t fold2(uint64_t a, uint64_t b, uint64_t r) {
     return fp61::add(a, fp61::mul(r, fp61::sub(b, a)));
@@ -72,30 +92,81 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 __device__ __forceinline__ void red_add(unsigned long long *p, unsigned long long v) {
     asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
+// barrier among the first nthr threads of the CTA (nthr a multiple of 32); id 1 (id 0 is __syncthreads)
+__device__ __forceinline__ void bar_n(uint32_t nthr) { asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory"); }
 
-// ---- grid rendezvous + all-reduce of K <= 64 canonical words (one per thread k < K, value in cx.acc[k]).
-// Every CTA adds (value & 2^32-1 | 1<<48) and (value >> 32 | 1<<48) into the slot of this epoch; a word is
-// complete when its count field equals the number of CTAs.  Totals land in cx.acc[k] of every CTA.
-// All global writes made by this CTA before the call are visible to every CTA after it (fence + acquire).
-__device__ __forceinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t K) {
+// Sum over the full warp of canonical words; every lane gets the canonical total.  Three integer warp reductions
+// (REDUX) on 27/27/7-bit pieces instead of five shuffle+add levels.
+__device__ __forceinline__ uint64_t warp_sum61(uint64_t v) {
+    uint32_t p0 = (uint32_t)v & 0x7ffffffu, p1 = (uint32_t)(v >> 27) & 0x7ffffffu, p2 = (uint32_t)(v >> 54);
+    p0 = __reduce_add_sync(0xffffffffu, p0);
+    p1 = __reduce_add_sync(0xffffffffu, p1);
+    p2 = __reduce_add_sync(0xffffffffu, p2);          // < 2^12
+    const uint64_t x = (uint64_t)p0 + ((uint64_t)p1 << 27) + ((uint64_t)(p2 & 127u) << 54) + (p2 >> 7);
+    return fp61::reduce62(x);                          // x < 2^32 + 2^59 + 2^61 + 32
+}
+
+// eq(u, x[k0..k1)) for one index u by direct product, two interleaved chains (no table, no barrier)
+__device__ __forceinline__ uint64_t eq_direct(uint32_t u, const uint64_t *x, uint32_t k0, uint32_t k1) {
+    uint64_t e0 = 1, e1 = 1;
+    uint32_t k = k0;
+    for (; k + 1 < k1; k += 2) {
+        e0 = fp61::mul(e0, fp61::chi((u >> (k - k0)) & 1u, x[k]));
+        e1 = fp61::mul(e1, fp61::chi((u >> (k + 1 - k0)) & 1u, x[k + 1]));
+    }
+    if (k < k1) e0 = fp61::mul(e0, fp61::chi((u >> (k - k0)) & 1u, x[k]));
+    return fp61::mul(e0, e1);
+}
+
+// Two-level eq table over variables x[0..nv): lo[u] = eq(u, x[0..cl)), hi[w] = eq(w, x[cl..ch)), cl = min(nv,10),
+// ch = min(nv,20); variables >= 20 are multiplied in per index by eq_of().  Threads [t0, t0+nthr) cooperate; the
+// caller provides the barrier afterwards.
+struct EqTab {
+    const uint64_t *lo, *hi, *x;
+    uint32_t nv;
+    __device__ __forceinline__ uint64_t eq_of(uint32_t u) const {
+        uint64_t e = lo[u & ((1u << F_EQLOG) - 1)];
+        if (nv > F_EQLOG) e = fp61::mul(e, hi[(u >> F_EQLOG) & ((1u << F_EQLOG) - 1)]);
+        if (nv > 2 * F_EQLOG) e = fp61::mul(e, eq_direct(u >> (2 * F_EQLOG), x, 2 * F_EQLOG, nv));
+        return e;
+    }
+};
+__device__ __forceinline__ EqTab build_eq_tab(uint64_t *lo, uint64_t *hi, const uint64_t *x, uint32_t nv, uint32_t t,
+                                              uint32_t nthr) {
+    const uint32_t cl = nv < F_EQLOG ? nv : F_EQLOG;
+    const uint32_t ch = nv < 2 * F_EQLOG ? nv : 2 * F_EQLOG;
+    for (uint32_t u = t; u < (1u << cl); u += nthr) lo[u] = eq_direct(u, x, 0, cl);
+    if (ch > cl)
+        for (uint32_t u = t; u < (1u << (ch - cl)); u += nthr) hi[u] = eq_direct(u, x, cl, ch);
+    EqTab e; e.lo = lo; e.hi = hi; e.x = x; e.nv = nv;
+    return e;
+}
+
+// ---- grid rendezvous + all-reduce of K <= 64 canonical words held in cx.acc[0..K) (CTA totals).
+// Every CTA adds (low 32 bits | 1<<48) and (high bits | 1<<48) into the slot of this epoch; a word is complete when
+// its count field equals the number of CTAs.  Totals land in cx.acc[k] of every CTA.  With fence = true all global
+// writes made by this CTA before the call are visible to every CTA after it.
+__device__ __forceinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t K, bool fence) {
     const uint32_t tid = threadIdx.x;
     __syncthreads();
-    unsigned long long *slot = a.slots + (size_t)(cx.epoch % F_RING) * F_SLOT_WORDS;
-    if (blockIdx.x == 0 && tid >= 128 && tid < 128 + F_SLOT_WORDS)   // recycle the slot of epoch+2
-        (a.slots + (size_t)((cx.epoch + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
+    const uint32_t ep = cx.epoch;
+    unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
+    if (blockIdx.x == 0 && tid >= 128 && tid < 128 + F_SLOT_WORDS) {  // recycle the slot of epoch+2
+        (a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
+        __threadfence();                 // ordered before CTA 0's post of epoch+1 (barrier below), hence before any post to it
+    }
     const uint32_t W = K == 0 ? 1 : 2 * K;
     uint64_t got = 0;
     if (tid < W) {
         const uint64_t v = K == 0 ? 0 : cx.acc[tid >> 1];
         const uint64_t part = (tid & 1) ? (v >> 32) : (v & 0xffffffffull);
-        __threadfence();
+        if (fence) __threadfence();
         red_add(slot + tid, part | F_CNT_ONE);
         const uint64_t want = (uint64_t)gridDim.x;
         unsigned long long w;
         while (((w = ld_acquire(slot + tid)) >> 48) != want) { }
         got = w & F_VAL_MASK;
     }
-    // combine lo + hi*2^32 (lo < 2^40, hi < 2^37)
     const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
     __syncthreads();
     if (tid < W && !(tid & 1) && K)
@@ -104,117 +175,41 @@ __device__ __forceinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a,
     __syncthreads();
 }
 
-// block-level sum of 3 words per thread -> cx.acc[0..2] on every thread's view (after the trailing barrier)
-__device__ __forceinline__ void block_reduce3(FusedCtx &cx, uint64_t (&v)[3]) {
-    block_sum<3>(v, cx.red);
-    if (threadIdx.x == 0) { cx.acc[0] = v[0]; cx.acc[1] = v[1]; cx.acc[2] = v[2]; }
+// ---- the per-round fast path: per-warp partials (3 words each) sit in cx.red[w*4 + k], w < nw.  Warp 0 combines
+// them, posts the CTA totals, polls, and leaves the grid totals in cx.G[0..2]; CTA 0 also writes them to tr.
+// Lane 0 then draws the challenge that answers this message, r = H(seed, ctr), into *rslot.  Two block barriers in all.
+__device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t nw, bool fence, uint64_t *tr,
+                                                uint64_t *rslot, uint64_t seed, uint32_t ctr) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    const uint32_t ep = cx.epoch;        // last written before the trailing barrier of the previous rendezvous
     __syncthreads();
-}
-
-// Elo[u] = eq(u, z[0..c)) for u < 2^c, by doubling (1 multiply per new entry); c <= 10.  Trailing barrier.
-__device__ __forceinline__ void build_eq_low(uint64_t *E, const uint64_t *z, uint32_t c) {
-    if (threadIdx.x == 0) E[0] = 1;
-    __syncthreads();
-    for (uint32_t k = 0; k < c; k++) {
-        const uint32_t half = 1u << k;
-        if (threadIdx.x < half) {
-            const uint64_t e = E[threadIdx.x], h = fp61::mul(e, z[k]);
-            E[threadIdx.x + half] = h;
-            E[threadIdx.x] = fp61::sub(e, h);
+    if (tid < 32) {
+        unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
+        const uint64_t t0 = warp_sum61(lane < nw ? cx.red[lane * 4 + 0] : 0);
+        const uint64_t t1 = warp_sum61(lane < nw ? cx.red[lane * 4 + 1] : 0);
+        const uint64_t t2 = warp_sum61(lane < nw ? cx.red[lane * 4 + 2] : 0);
+        uint64_t got = 0;
+        if (lane < 6) {
+            const uint64_t v = lane < 2 ? t0 : (lane < 4 ? t1 : t2);
+            const uint64_t part = (lane & 1) ? (v >> 32) : (v & 0xffffffffull);
+            if (fence) __threadfence();
+            red_add(slot + lane, part | F_CNT_ONE);
+            const uint64_t want = (uint64_t)gridDim.x;
+            unsigned long long w;
+            while (((w = ld_acquire(slot + lane)) >> 48) != want) { }
+            got = w & F_VAL_MASK;
         }
-        __syncthreads();
-    }
-}
-
-// ---- a7, fused: cx.acc[t-2] <- sum over this CTA's share of V_{i+1} of eq(u, l(t)) V[u],  t = 2..s.
-// One pass over the CTA's virtual blocks (2^(3+tb) words each, tb = min(s-3,10) thread bits): a thread folds its 8
-// words with l(t)_{0..2}, weights by eq(lane bits), the warp sum is weighted by eq(warp bits, block bits).
-// scratch: pts[m*s] | Wl[m*32] | Ww[m*32] | red[m*32]   (m = s-1 <= 63)
-__device__ __forceinline__ void line_partials(const uint64_t *__restrict__ Vb, uint32_t s, FusedCtx &cx, uint64_t *scratch,
-                                              uint32_t vb0, uint32_t vbstride) {
-    const uint32_t m = s - 1, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint64_t *pts = scratch, *Wl = pts + (size_t)m * s, *Ww = Wl + (size_t)m * 32, *red = Ww + (size_t)m * 32;
-    const uint32_t nt = s < 3 ? s : 3;
-    const uint32_t tb = (s - nt) < 10 ? (s - nt) : 10;
-    const uint32_t lb = tb < 5 ? tb : 5, wb = tb - lb;
-    const uint32_t nvb = 1u << (s - nt - tb);
-    if (tid < m) cx.acc[tid] = 0;
-    for (uint32_t i = tid; i < m * s; i += FT) {
-        const uint32_t t = i / s + 2, k = i % s;
-        pts[i] = fp61::add(cx.r1[k], fp61::mul(t, fp61::sub(cx.r2[k], cx.r1[k])));
-    }
-    __syncthreads();
-    // lane tables do not depend on the block: Wl[t][l] = eq(l, pts[t][nt..nt+lb))
-    for (uint32_t i = tid; i < m * 32; i += FT) {
-        const uint32_t t = i >> 5, l = i & 31;
-        uint64_t e = 1;
-        for (uint32_t k = 0; k < lb; k++) e = fp61::mul(e, fp61::chi((l >> k) & 1u, pts[t * s + nt + k]));
-        Wl[i] = (l < (1u << lb)) ? e : 0;
-    }
-    const bool active = tid < (1u << tb);
-    for (uint32_t vb = vb0; vb < nvb; vb += vbstride) {
-        __syncthreads();
-        for (uint32_t i = tid; i < m * 32; i += FT) {   // Ww[t][w] = eq(w, warp bits) * eq(vb, block bits)
-            const uint32_t t = i >> 5, w = i & 31;
-            uint64_t e = 1;
-            for (uint32_t k = 0; k < wb; k++) e = fp61::mul(e, fp61::chi((w >> k) & 1u, pts[t * s + nt + lb + k]));
-            for (uint32_t k = nt + tb; k < s; k++) e = fp61::mul(e, fp61::chi((vb >> (k - nt - tb)) & 1u, pts[t * s + k]));
-            Ww[i] = e;
+        const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
+        if (lane < 6 && !(lane & 1)) {
+            const uint64_t g = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
+            cx.G[lane >> 1] = g;
+            if (blockIdx.x == 0) tr[lane >> 1] = g;
         }
-        uint64_t v[8];
-        const size_t base = (((size_t)vb << tb) + tid) << nt;
-#pragma unroll
-        for (int e = 0; e < 8; e++) v[e] = (active && e < (1 << nt)) ? Vb[base + e] : 0;
-        __syncthreads();
-        for (uint32_t t = 0; t < m; t++) {
-            uint64_t f[8];
-#pragma unroll
-            for (int e = 0; e < 8; e++) f[e] = v[e];
-#pragma unroll
-            for (int k = 0; k < 3; k++) {
-                if (k < (int)nt) {
-                    const uint64_t x = pts[t * s + k];
-#pragma unroll
-                    for (int e = 0; e < (8 >> (k + 1)); e++) f[e] = fold2(f[2 * e], f[2 * e + 1], x);
-                }
-            }
-            uint64_t val = active ? fp61::mul(f[0], Wl[t * 32 + lane]) : 0;
-            val = warp_sum(val);
-            if (lane == 0) red[t * 32 + warp] = fp61::mul(val, Ww[t * 32 + warp]);
-        }
-        __syncthreads();
-        if (tid < m) {
-            uint64_t acc = cx.acc[tid];
-            const uint32_t nw = active ? ((1u << tb) + 31) >> 5 : 0;
-            for (uint32_t w = 0; w < (((1u << tb) + 31) >> 5); w++) acc = fp61::add(acc, red[tid * 32 + w]);
-            (void)nw;
-            cx.acc[tid] = acc;
-        }
+        if (lane == 0) { cx.epoch = ep + 1; *rslot = fp61::draw(seed, ctr); }
+    } else if (blockIdx.x == 0 && tid >= 128 && tid < 128 + F_SLOT_WORDS) {
+        (a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
+        __threadfence();
     }
-    __syncthreads();
-}
-
-// after the totals q[2..s] sit in cx.acc[0..m): write q, draw tau, z <- l(tau), claim <- q(tau).  All CTAs run it
-// (identical results); only `writer` stores the transcript.
-__device__ __forceinline__ void line_finish(uint32_t s, FusedCtx &cx, const DevState *st, uint64_t *tr_q, bool writer) {
-    const uint32_t tid = threadIdx.x;
-    if (tid <= s) cx.q[tid] = tid == 0 ? cx.v1 : (tid == 1 ? cx.v2 : cx.acc[tid - 2]);
-    __syncthreads();
-    const uint64_t tau = fp61::draw(cx.seed, cx.ctr);
-    if (writer && tid <= s) tr_q[tid] = cx.q[tid];
-    uint64_t term = 0;
-    if (tid <= s) {
-        uint64_t num = 1;
-        for (uint32_t mm = 0; mm <= s; mm++)
-            if (mm != tid) num = fp61::mul(num, fp61::sub(tau, mm));
-        const uint64_t dinv = fp61::mul(st->invfact[tid], st->invfact[s - tid]);
-        term = fp61::mul(cx.q[tid], fp61::mul(num, dinv));
-        if ((s - tid) & 1u) term = fp61::neg(term);
-    }
-    uint64_t tv[1] = {term};
-    block_sum<1>(tv, cx.red);
-    if (tid < s) cx.z[tid] = fold2(cx.r1[tid], cx.r2[tid], tau);
-    if (tid == 0) { cx.claim = tv[0]; cx.ctr += 1; }
     __syncthreads();
 }
 

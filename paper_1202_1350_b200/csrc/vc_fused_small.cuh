@@ -1,63 +1,136 @@
 // vc_fused_small.cuh — one narrow layer (<= 2^10 gates, table <= 2^12 words) proved by a single CTA out of shared
-// memory: one gate per thread in registers, fold tables in shared memory, block barriers only (steps a2-a7).
+// memory (steps a2-a7).  One gate per thread in registers; only as many warps as the layer needs take part and they
+// synchronise on a named barrier, so a round of a 1-gate layer costs two 1-warp barriers, not two 32-warp ones.
+// Per round: contributions -> 3 warp REDUX sums -> barrier (message complete) -> challenge -> weight update and
+// table fold -> barrier.  Warp 0 sums the per-warp partials and writes the transcript off the critical path.
 #pragma once
 #include "vc_fused.cuh"
+#include "vc_fused_line.cuh"
 
 namespace vc {
 
-__device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, uint8_t *dyn, uint32_t layer, uint64_t *tr) {
-    const uint32_t tid = threadIdx.x;
-    const LayerDesc Li = a.L[layer], Lb = a.L[layer + 1];
-    const uint32_t si = Li.log_n, s = Lb.log_n;
-    const uint32_t n = 1u << si, nb = 1u << s;
-    uint64_t *Vs = reinterpret_cast<uint64_t *>(dyn);           // V_{i+1}, 2^s words
-    uint64_t *A0 = Vs + (1u << F_SMALL_T_LOG);                   // fold ping-pong: 2^(s-1), 2^(s-2)
-    uint64_t *A1 = A0 + (1u << (F_SMALL_T_LOG - 1));
-    uint64_t *E = A1 + (1u << (F_SMALL_T_LOG - 2));              // beta table, 2^si words
-    uint64_t *scratch = E + (1u << F_SMALL_N_LOG);               // line restriction scratch
-    for (uint32_t u = tid; u < nb; u += FT) Vs[u] = Lb.V[u];
-    build_eq_low(E, cx.z, si);                                   // a3 (trailing barrier covers Vs too)
-    const bool live = tid < n;
-    uint64_t Pg = live ? E[tid] : 0;
-    uint32_t i1 = 0, i2 = 0, t = 3;
-    if (live) { i1 = Li.in1[tid]; i2 = Li.in2[tid]; t = Li.type[tid]; }
-    const uint64_t w = Vs[i2];
-    if (layer == 0) {                                            // a2
-        uint64_t v[3] = {live ? fp61::mul(Pg, Li.V[tid]) : 0, 0, 0};
-        block_reduce3(cx, v);
-        if (tid == 0) cx.claim = cx.acc[0];
-    }
-    for (int phase = 1; phase <= 2; phase++) {
-        const uint32_t idx = phase == 1 ? i1 : i2;
-        const uint64_t *tab = Vs;
-        for (uint32_t j = 0; j < s; j++) {
-            acc128 a0, a1, a2; a0.clear(); a1.clear(); a2.clear();
-            const uint32_t bit = (idx >> j) & 1u, u = idx >> (j + 1);
-            const uint64_t lo = tab[2 * u], hi = tab[2 * u + 1];
-            if (phase == 1) gate_terms<1>(t, Pg, w, bit, lo, hi, a0, a1, a2);
-            else gate_terms<2>(t, Pg, cx.v1, bit, lo, hi, a0, a1, a2);
-            uint64_t v3[3] = {a0.value(), a1.value(), a2.value()};
-            block_reduce3(cx, v3);
-            const uint64_t r = fp61::draw(cx.seed, cx.ctr);
-            if (tid < 3) tr[tid] = cx.acc[tid];
-            tr += 3;
-            Pg = fp61::mul(Pg, bit ? r : fp61::sub(1, r));       // a6
-            uint64_t *out = (j & 1) ? A1 : A0;
-            const uint32_t half = nb >> (j + 1);
-            for (uint32_t v = tid; v < half; v += FT) out[v] = fold2(tab[2 * v], tab[2 * v + 1], r);
-            __syncthreads();
-            if (tid == 0) { cx.ctr += 1; if (phase == 1) cx.r1[j] = r; else cx.r2[j] = r; }
-            tab = out;
-        }
-        if (tid == 0) { if (phase == 1) cx.v1 = tab[0]; else cx.v2 = tab[0]; }
-        __syncthreads();
-    }
-    if (s > 1) line_partials(Lb.V, s, cx, scratch, 0, 1);
-    line_finish(s, cx, a.st, tr, true);
+constexpr size_t F_SMALL_WORDS = (1u << F_SMALL_T_LOG) + (1u << (F_SMALL_T_LOG - 1)) + (1u << (F_SMALL_T_LOG - 2)) + 2 * 32 * 4;
+
+// per-type (W, c, ignore-x) of a gate for a phase:  contribution = W * (x + c)   (x := 0 when ignore)
+//   phase 1 (x = V~(w1) side, other = V[in2]):  MULT (P*other, 0)  ADD (P, other)  SUB (P, -other)  RELAY (P, 0)
+//   phase 2 (x = V~(w2) side, other = v1):      MULT (P*v1, 0)     ADD (P, v1)     SUB (-P, -v1)    RELAY (P, v1; x ignored)
+__device__ __forceinline__ void gate_state(int phase, uint32_t t, uint64_t P, uint64_t other, uint64_t &W, uint64_t &c,
+                                           uint32_t &ign) {
+    ign = 0;
+    if (t == VC_MULT) { W = fp61::mul(P, other); c = 0; }
+    else if (t == VC_ADD) { W = P; c = other; }
+    else if (t == VC_SUB) { W = phase == 1 ? P : fp61::neg(P); c = fp61::neg(other); }
+    else { W = P; c = phase == 1 ? 0 : other; ign = phase == 1 ? 0u : 1u; }
 }
 
-constexpr size_t F_SMALL_BYTES = ((1u << F_SMALL_T_LOG) + (1u << (F_SMALL_T_LOG - 1)) + (1u << (F_SMALL_T_LOG - 2)) +
-                                  (1u << F_SMALL_N_LOG)) * 8 + (64 * 64 + 3 * 64 * 32) * 8;
-static_assert(F_SMALL_BYTES <= F_STATE_BYTES, "small-layer buffers alias the gate-state region");
+// One gate's two products of a round, accumulated without reduction:
+//   X += W (x_b + c)      and, if b, X1 += the same           ->  G[0] = X - X1,  G[1] = X1
+//   Y += W (x_2 + c)      and, if b, Y1 += the same           ->  G[2] = 2 Y1 - (Y - Y1)      (chi(1,2) = 2, chi(0,2) = -1)
+// with x_b = b ? hi : lo and x_2 = 2 hi - lo.  Operands stay below 2^63, products below 2^124: 8 of them fit 128 bits.
+__device__ __forceinline__ void gate_mac(uint64_t W, uint64_t c, uint32_t b, uint64_t lo, uint64_t hi, acc128 &X, acc128 &X1,
+                                         acc128 &Y, acc128 &Y1) {
+    const uint64_t mb = (b ? hi : lo) + c;                       // < 2^62
+    const uint64_t m2 = 2 * hi + (fp61::P - lo) + c;             // < 2^63
+    const uint64_t msk = 0ull - (uint64_t)b;
+    uint64_t pl = W * mb, ph = fp61::mulhi(W, mb);
+    X.lo += pl; X.hi += ph + (X.lo < pl);
+    pl &= msk; ph &= msk;
+    X1.lo += pl; X1.hi += ph + (X1.lo < pl);
+    pl = W * m2; ph = fp61::mulhi(W, m2);
+    Y.lo += pl; Y.hi += ph + (Y.lo < pl);
+    pl &= msk; ph &= msk;
+    Y1.lo += pl; Y1.hi += ph + (Y1.lo < pl);
+}
+__device__ __forceinline__ void gate_fin(const acc128 &X, const acc128 &X1, const acc128 &Y, const acc128 &Y1, uint64_t (&g)[3]) {
+    const uint64_t x = X.value(), x1 = X1.value(), y = Y.value(), y1 = Y1.value();
+    g[0] = fp61::sub(x, x1);
+    g[1] = x1;
+    g[2] = fp61::sub(fp61::add(fp61::dbl(y1), y1), y);
+}
+
+__device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, uint8_t *dyn,
+                                            uint32_t layer, uint64_t *tr) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t si = a.L[layer].log_n, s = a.L[layer + 1].log_n;
+    const uint32_t n = 1u << si, nb = 1u << s;
+    uint32_t nthr = 32;
+    { const uint32_t need = n > (nb >> 1) ? n : (nb >> 1); while (nthr < need && nthr < (uint32_t)FT) nthr <<= 1; }
+    __syncthreads();                                             // bookkeeping of the previous layer is settled
+    if (tid < nthr) {
+        uint64_t *Vs = reinterpret_cast<uint64_t *>(dyn);        // level 0: V_{i+1}
+        uint64_t *X = Vs + (1u << F_SMALL_T_LOG);                 // odd levels
+        uint64_t *Y = X + (1u << (F_SMALL_T_LOG - 1));            // even levels >= 2
+        uint64_t *sred = Y + (1u << (F_SMALL_T_LOG - 2));         // [parity][warp][4]
+        uint64_t *scratch = sred + 2 * 32 * 4;
+        const uint32_t nw = nthr >> 5;
+        const uint64_t *Vg = a.L[layer + 1].V;
+        for (uint32_t u = tid; u < nb; u += nthr) Vs[u] = Vg[u];
+        const bool live = tid < n;
+        uint64_t P = live ? eq_direct(tid, cx.z, 0, si) : 0;     // a3: beta(z, g) by direct product
+        uint32_t i1 = 0, i2 = 0, t = VC_RELAY;
+        if (live) { i1 = a.L[layer].in1[tid]; i2 = a.L[layer].in2[tid]; t = a.L[layer].type[tid]; }
+        uint32_t ctr = (uint32_t)cx.ctr;
+        const uint64_t seed = cx.seed;
+        bar_n(nthr);
+        if (layer == 0) {                                        // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
+            const uint64_t v = warp_sum61(live ? fp61::mul(P, a.L[0].V[tid]) : 0);
+            if (lane == 0) sred[warp * 4] = v;
+            bar_n(nthr);
+            if (warp == 0) {
+                const uint64_t tot = warp_sum61(lane < nw ? sred[lane * 4] : 0);
+                if (lane == 0) cx.claim = tot;
+            }
+            bar_n(nthr);
+        }
+        uint32_t par = 0;
+        for (int phase = 1; phase <= 2; phase++) {
+            const uint32_t idx = phase == 1 ? i1 : i2;
+            uint64_t W, c; uint32_t ign;
+            gate_state(phase, t, P, phase == 1 ? Vs[i2] : cx.v1, W, c, ign);
+            if (!live) { W = 0; c = 0; }
+            for (uint32_t j = 0; j < s; j++) {
+                const uint64_t *tab = j == 0 ? Vs : ((j & 1) ? X : Y);
+                const uint32_t bit = (idx >> j) & 1u, u = idx >> (j + 1);
+                uint64_t lo = tab[2 * u], hi = tab[2 * u + 1];
+                if (ign) { lo = 0; hi = 0; }
+                acc128 A, A1, B, B1; A.clear(); A1.clear(); B.clear(); B1.clear();
+                gate_mac(W, c, bit, lo, hi, A, A1, B, B1);
+                uint64_t g[3];
+                gate_fin(A, A1, B, B1, g);
+                uint64_t *pr = sred + par * 128;
+#pragma unroll
+                for (int k = 0; k < 3; k++) { g[k] = warp_sum61(g[k]); if (lane == 0) pr[warp * 4 + k] = g[k]; }
+                bar_n(nthr);                                     // the message of this round is complete
+                if (warp == 0) {                                 // transcript, off the critical path of the other warps
+#pragma unroll
+                    for (int k = 0; k < 3; k++) {
+                        const uint64_t tot = warp_sum61(lane < nw ? pr[lane * 4 + k] : 0);
+                        if (lane == 0) tr[k] = tot;
+                    }
+                }
+                tr += 3; par ^= 1;
+                const uint64_t r = fp61::draw(seed, ctr); ctr++;   // a6: challenge, weight update, fold
+                const uint64_t f = bit ? r : fp61::sub(1, r);
+                W = fp61::mul(W, f); P = fp61::mul(P, f);
+                uint64_t *out = ((j + 1) & 1) ? X : Y;
+                const uint32_t half = nb >> (j + 1);
+                for (uint32_t v = tid; v < half; v += nthr) out[v] = fold2(tab[2 * v], tab[2 * v + 1], r);
+                if (tid == 0) { if (phase == 1) cx.r1[j] = r; else cx.r2[j] = r; }
+                bar_n(nthr);
+            }
+            const uint64_t vend = ((s & 1) ? X : Y)[0];           // level s: V~_{i+1}(r1) resp. (r2)
+            if (tid == 0) { if (phase == 1) cx.v1 = vend; else cx.v2 = vend; }
+            // P now equals beta(z,g) eq(in1[g], r1): the plain weight phase 2 starts from
+            bar_n(nthr);
+        }
+        if (tid == 0) cx.ctr = ctr;
+        if (s > 1) line_partials(Vs, s, cx, scratch, 0, 1, tid, nthr);   // a7 (its first barrier publishes cx.ctr)
+        else bar_n(nthr);
+        line_finish(s, cx, invfact, tr, true, tid);
+    }
+    __syncthreads();
+}
+
+constexpr size_t F_SMALL_BYTES = (F_SMALL_WORDS + 11 * 12 + 3 * 11 * 32) * 8;
 
 }  // namespace vc
