@@ -99,6 +99,9 @@ int vc_debug_state(const vc_circuit *c, uint64_t *h_z64, uint64_t *h_claim, uint
 int vc_debug_values(const vc_circuit *c, uint32_t layer, uint64_t *h_values, void *cuda_stream);
 /* fused schedule only: d+1 device timestamps (ns, %globaltimer): start of each layer's proof, [d] = end */
 int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *cuda_stream);
+/* fused schedule, builds with -DVC_TRACE only (all zero otherwise): the first n_words <= 65536 trace words of the last
+ * launch, each (code << 48 | SM clock of CTA 0) */
+int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, void *cuda_stream);
 /* sticky device-side status: 0 = fine, 1 = a non-canonical input word was seen by vc_evaluate */
 int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */

@@ -15,7 +15,7 @@ EXPORTS = [
     "vc_circuit_load", "vc_evaluate", "vc_prove_layer", "vc_prove", "vc_run_host", "vc_verify_transcript",
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
-    "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps",
+    "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
 ]
 
 
@@ -66,6 +66,7 @@ def lib():
             "vc_debug_fieldop": (i32, [i32, vp, vp, vp, u64, vp]),
             "vc_bench_modmul": (i32, [u32, u32, u32, u32, vp, vp]),
             "vc_debug_layer_stamps": (i32, [vp, vp, vp]),
+            "vc_debug_trace": (i32, [vp, vp, u32, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
         }

@@ -63,6 +63,20 @@ struct acc128 {
     __host__ __device__ __forceinline__ uint64_t value() const { return fold128(hi, lo); }
 };
 
+#ifdef __CUDACC__
+// (lo,hi) += a*b, and, if pred, (lo1,hi1) += a*b too: one 64x64->128 product, two carry-chain adds (the second predicated)
+__device__ __forceinline__ void mac2(uint64_t &lo, uint64_t &hi, uint64_t &lo1, uint64_t &hi1, uint64_t a, uint64_t b,
+                                     uint32_t pred) {
+    asm("{\n\t.reg .u64 pl, ph;\n\t.reg .pred p;\n\t"
+        "setp.ne.u32 p, %6, 0;\n\t"
+        "mul.lo.u64 pl, %4, %5;\n\tmul.hi.u64 ph, %4, %5;\n\t"
+        "add.cc.u64 %0, %0, pl;\n\taddc.u64 %1, %1, ph;\n\t"
+        "@p add.cc.u64 %2, %2, pl;\n\t@p addc.u64 %3, %3, ph;\n\t}"
+        : "+l"(lo), "+l"(hi), "+l"(lo1), "+l"(hi1)
+        : "l"(a), "l"(b), "r"(pred));
+}
+#endif
+
 // chi(b, x) = x if b else 1 - x
 __host__ __device__ __forceinline__ uint64_t chi(uint32_t b, uint64_t x) { return b ? x : sub(1, x); }
 

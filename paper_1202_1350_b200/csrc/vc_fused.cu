@@ -24,13 +24,14 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (tid == 0) { cx.seed = a.seed; cx.ctr = a.st->ctr; cx.claim = a.st->claim; }
     }
     if (tid <= MAX_VARS) invfact[tid] = a.st->invfact[tid];
-    if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; }
+    if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; cx.pad = 0; cx.pend_tr = nullptr; cx.pend_slot = 0; }
     __syncthreads();
     uint64_t *tr = a.tr;
     bool handoff = false;                         // CTA 0 ran narrow layers alone: publish its state first
     for (uint32_t layer = a.begin; layer < a.end; layer++) {
         const uint32_t s = a.L[layer + 1].log_n;
         if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
+        VC_TR(100 + layer);
         if (a.L[layer].kind == 0) {
             if (blockIdx.x == 0) small_layer(a, cx, invfact, dyn, layer, tr);
             handoff = true;
@@ -134,7 +135,6 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         const size_t st_bytes = res ? state : 0;
         const size_t total = F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8;
         if (total > F_SMEM_MAX) continue;
-        if (res && cap > 8u * FT) continue;      // accumulators hold 8 products between reductions either way; keep the resident loop short
         lp.resident = res ? 1 : 0;
         lp.cap = (uint32_t)cap;
         for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = use[ph] ? F_MODE_SLICE : F_MODE_GLOBAL; lp.K[ph] = K; }
@@ -184,11 +184,11 @@ int fused_init(vc_circuit *c) {
     if (cudaMalloc(&fh.d_plan, h.size() * sizeof(LayerPlan)) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_cta, std::max<size_t>(all_cta.size(), 1) * sizeof(CtaPlan)) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_slots, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_NOMEM;
-    if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_C, max_gates * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_Tg, (size_t)(2u << F_TLOG) * 8) != cudaSuccess) return VC_ERR_NOMEM;
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
-    if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1) * 8) != cudaSuccess) return VC_ERR_CUDA;
+    if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (!all_cta.empty() &&
         cudaMemcpy(fh.d_cta, all_cta.data(), all_cta.size() * sizeof(CtaPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
@@ -231,6 +231,13 @@ int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st) {
     if (!fh) return VC_ERR_STATE;
     if (cudaStreamSynchronize(st) != cudaSuccess) return VC_ERR_CUDA;
     return cudaMemcpy(h, fh->d_stamps, (size_t)(c->d + 1) * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? VC_OK : VC_ERR_CUDA;
+}
+
+int fused_trace(const vc_circuit *c, uint64_t *h, uint32_t n_words, cudaStream_t st) {
+    FusedHost *fh = find(c);
+    if (!fh || n_words > F_TRACE_WORDS) return VC_ERR_ARG;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return VC_ERR_CUDA;
+    return cudaMemcpy(h, fh->d_stamps + c->d + 1, (size_t)n_words * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? VC_OK : VC_ERR_CUDA;
 }
 
 int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {

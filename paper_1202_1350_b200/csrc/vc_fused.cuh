@@ -19,10 +19,10 @@
 
 namespace vc {
 
-constexpr int FT = 1024;                 // threads per CTA
+constexpr int FT = 512;                  // threads per CTA (128 registers each)
 constexpr int F_TLOG = 10;               // the fully shared part of a fold table has 2^min(s, F_TLOG) entries
 constexpr int F_EQLOG = 10;              // eq tables are built in halves of at most 2^10 entries
-constexpr int F_SMALL_N_LOG = 10;        // single-CTA path: gates <= 2^10 ...
+constexpr int F_SMALL_N_LOG = 9;         // single-CTA path: gates <= 2^9 (one per thread) ...
 constexpr int F_SMALL_T_LOG = 12;        // ... and table <= 2^12 words
 constexpr int F_SLOT_WORDS = 128;        // one rendezvous slot: up to 64 values x (lo,hi)
 constexpr int F_RING = 4;
@@ -71,10 +71,27 @@ struct FusedCtx {            // block-shared bookkeeping, replicated in every CT
     uint64_t G[4];
     uint64_t seed, ctr, claim, v1, v2;
     uint32_t epoch, pad;
+    uint64_t *pend_tr;       // CTA 0: transcript position of the round whose slot is not converted yet (or null)
+    uint32_t pend_slot, pad2;
 };
 
 // fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS; the rest starts 16-byte aligned
 constexpr size_t F_FIXED_BYTES = (sizeof(FusedCtx) + (MAX_VARS + 1) * 8 + 15) & ~(size_t)15;
+
+// Optional fine-grained trace (compile with -DVC_TRACE): CTA 0 / thread 0 appends (code << 48 | SM clock) after the
+// d+1 layer stamps; read back with vc_debug_layer_stamps' buffer via vc_debug_trace.  Off in the product build.
+constexpr uint32_t F_TRACE_WORDS = 1u << 16;
+#ifdef VC_TRACE
+#define VC_TR(code)                                                                                          \
+    do {                                                                                                     \
+        if (blockIdx.x == 0 && threadIdx.x == 0 && cx.pad < F_TRACE_WORDS) {                                 \
+            a.stamps[a.d + 1 + cx.pad] = ((uint64_t)(code) << 48) | ((uint64_t)clock64() & 0xffffffffffffull); \
+            cx.pad++;                                                                                        \
+        }                                                                                                    \
+    } while (0)
+#else
+#define VC_TR(code) do { } while (0)
+#endif
 
 __device__ __forceinline__ uint64_t fold2(uint64_t a, uint64_t b, uint64_t r) {
     return fp61::add(a, fp61::mul(r, fp61::sub(b, a)));
@@ -176,8 +193,40 @@ __device__ __forceinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a,
 }
 
 // ---- the per-round fast path: per-warp partials (3 words each) sit in cx.red[w*4 + k], w < nw.  Warp 0 combines
-// them, posts the CTA totals, polls, and leaves the grid totals in cx.G[0..2]; CTA 0 also writes them to tr.
-// Lane 0 then draws the challenge that answers this message, r = H(seed, ctr), into *rslot.  Two block barriers in all.
+// them and posts the CTA totals as six (value | count) words; lane 0 alone waits until word 0 carries every CTA's
+// count: that is the rendezvous ("message complete").  Nobody needs the grid totals to go on, so they are not read
+// back here: warp 2 of CTA 0 turns the slot of the PREVIOUS round into transcript words while the next round runs
+// (transcript_flush does it for the last round of a phase).  The challenge that answers the message, r = H(seed,
+// ctr), is generated by warp 0 while it waits and handed out through *rslot only after the rendezvous.
+__device__ __forceinline__ unsigned long long atom_add(unsigned long long *p, unsigned long long v) {
+    unsigned long long r;
+    asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(r) : "l"(p), "l"(v) : "memory");
+    return r;
+}
+__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+// converts a completed slot (6 words) into G[0..2] -> tr[0..2]; called by one full warp of CTA 0
+__device__ __forceinline__ void slot_to_transcript(const unsigned long long *slot, uint64_t *tr, uint32_t lane) {
+    uint64_t got = 0;
+    if (lane < 6) {
+        const uint64_t want = (uint64_t)gridDim.x;
+        unsigned long long w;
+        while (((w = ld_relaxed(slot + lane)) >> 48) != want) { }
+        got = w & F_VAL_MASK;
+    }
+    const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
+    if (lane < 6 && !(lane & 1)) tr[lane >> 1] = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
+}
+__device__ __forceinline__ void transcript_flush(FusedCtx &cx, const FusedArgs &a) {   // CTA 0, warp 2 only
+    if (cx.pend_tr) {
+        slot_to_transcript(a.slots + (size_t)cx.pend_slot * F_SLOT_WORDS, cx.pend_tr, threadIdx.x & 31);
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) cx.pend_tr = nullptr;
+    }
+}
 __device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t nw, bool fence, uint64_t *tr,
                                                 uint64_t *rslot, uint64_t seed, uint32_t ctr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31;
@@ -188,27 +237,29 @@ __device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a
         const uint64_t t0 = warp_sum61(lane < nw ? cx.red[lane * 4 + 0] : 0);
         const uint64_t t1 = warp_sum61(lane < nw ? cx.red[lane * 4 + 1] : 0);
         const uint64_t t2 = warp_sum61(lane < nw ? cx.red[lane * 4 + 2] : 0);
-        uint64_t got = 0;
+        const uint64_t r = fp61::draw(seed, ctr);
         if (lane < 6) {
             const uint64_t v = lane < 2 ? t0 : (lane < 4 ? t1 : t2);
-            const uint64_t part = (lane & 1) ? (v >> 32) : (v & 0xffffffffull);
+            const uint64_t part = ((lane & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE;
             if (fence) __threadfence();
-            red_add(slot + lane, part | F_CNT_ONE);
-            const uint64_t want = (uint64_t)gridDim.x;
-            unsigned long long w;
-            while (((w = ld_acquire(slot + lane)) >> 48) != want) { }
-            got = w & F_VAL_MASK;
+            if (lane == 0) {
+                const uint64_t want = (uint64_t)gridDim.x;
+                if ((atom_add(slot, part) >> 48) + 1 != want)
+                    while ((ld_relaxed(slot) >> 48) != want) { }
+                if (fence) __threadfence();
+            } else {
+                red_add(slot + lane, part);
+            }
         }
-        const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
-        if (lane < 6 && !(lane & 1)) {
-            const uint64_t g = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
-            cx.G[lane >> 1] = g;
-            if (blockIdx.x == 0) tr[lane >> 1] = g;
+        if (lane == 0) { cx.epoch = ep + 1; *rslot = r; }
+    } else if (blockIdx.x == 0) {
+        if (tid >= 64 && tid < 96) {     // transcript of the previous round, then remember this one
+            transcript_flush(cx, a);
+            if (lane == 0) { cx.pend_slot = ep % F_RING; cx.pend_tr = tr; }
+        } else if (tid >= 128 && tid < 128 + F_SLOT_WORDS) {
+            (a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
+            __threadfence();
         }
-        if (lane == 0) { cx.epoch = ep + 1; *rslot = fp61::draw(seed, ctr); }
-    } else if (blockIdx.x == 0 && tid >= 128 && tid < 128 + F_SLOT_WORDS) {
-        (a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
-        __threadfence();
     }
     __syncthreads();
 }

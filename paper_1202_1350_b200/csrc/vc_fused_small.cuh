@@ -31,15 +31,8 @@ __device__ __forceinline__ void gate_mac(uint64_t W, uint64_t c, uint32_t b, uin
                                          acc128 &Y, acc128 &Y1) {
     const uint64_t mb = (b ? hi : lo) + c;                       // < 2^62
     const uint64_t m2 = 2 * hi + (fp61::P - lo) + c;             // < 2^63
-    const uint64_t msk = 0ull - (uint64_t)b;
-    uint64_t pl = W * mb, ph = fp61::mulhi(W, mb);
-    X.lo += pl; X.hi += ph + (X.lo < pl);
-    pl &= msk; ph &= msk;
-    X1.lo += pl; X1.hi += ph + (X1.lo < pl);
-    pl = W * m2; ph = fp61::mulhi(W, m2);
-    Y.lo += pl; Y.hi += ph + (Y.lo < pl);
-    pl &= msk; ph &= msk;
-    Y1.lo += pl; Y1.hi += ph + (Y1.lo < pl);
+    fp61::mac2(X.lo, X.hi, X1.lo, X1.hi, W, mb, b);
+    fp61::mac2(Y.lo, Y.hi, Y1.lo, Y1.hi, W, m2, b);
 }
 __device__ __forceinline__ void gate_fin(const acc128 &X, const acc128 &X1, const acc128 &Y, const acc128 &Y1, uint64_t (&g)[3]) {
     const uint64_t x = X.value(), x1 = X1.value(), y = Y.value(), y1 = Y1.value();
@@ -83,6 +76,7 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
             bar_n(nthr);
         }
         uint32_t par = 0;
+        VC_TR(1);
         for (int phase = 1; phase <= 2; phase++) {
             const uint32_t idx = phase == 1 ? i1 : i2;
             uint64_t W, c; uint32_t ign;
@@ -100,7 +94,9 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
                 uint64_t *pr = sred + par * 128;
 #pragma unroll
                 for (int k = 0; k < 3; k++) { g[k] = warp_sum61(g[k]); if (lane == 0) pr[warp * 4 + k] = g[k]; }
+                VC_TR(2);
                 bar_n(nthr);                                     // the message of this round is complete
+                VC_TR(3);
                 if (warp == 0) {                                 // transcript, off the critical path of the other warps
 #pragma unroll
                     for (int k = 0; k < 3; k++) {
@@ -116,7 +112,9 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
                 const uint32_t half = nb >> (j + 1);
                 for (uint32_t v = tid; v < half; v += nthr) out[v] = fold2(tab[2 * v], tab[2 * v + 1], r);
                 if (tid == 0) { if (phase == 1) cx.r1[j] = r; else cx.r2[j] = r; }
+                VC_TR(4);
                 bar_n(nthr);
+                VC_TR(5);
             }
             const uint64_t vend = ((s & 1) ? X : Y)[0];           // level s: V~_{i+1}(r1) resp. (r2)
             if (tid == 0) { if (phase == 1) cx.v1 = vend; else cx.v2 = vend; }
@@ -124,9 +122,12 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
             bar_n(nthr);
         }
         if (tid == 0) cx.ctr = ctr;
+        VC_TR(6);
         if (s > 1) line_partials(Vs, s, cx, scratch, 0, 1, tid, nthr);   // a7 (its first barrier publishes cx.ctr)
         else bar_n(nthr);
+        VC_TR(7);
         line_finish(s, cx, invfact, tr, true, tid);
+        VC_TR(8);
     }
     __syncthreads();
 }

@@ -49,7 +49,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;
     const uint32_t nk = (ng + FT - 1) / FT;
-    const uint32_t nw = ng >= (uint32_t)FT ? 32u : (ng + 31) / 32;   // warps that own gates
+    const uint32_t nw = ng >= (uint32_t)FT ? (uint32_t)FT / 32 : (ng + 31) / 32;   // warps that own gates
     const uint32_t cap = Lp.cap;
     uint64_t *sW = reinterpret_cast<uint64_t *>(dyn);
     uint64_t *sC = sW + cap;
@@ -79,11 +79,12 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
         claim_part = warp_sum61(claim_part);
         if (lane == 0) cx.red[warp * 4] = claim_part;
         __syncthreads();
-        if (warp == 0) { const uint64_t t0 = warp_sum61(cx.red[lane * 4]); if (lane == 0) cx.acc[0] = t0; }
+        if (warp == 0) { const uint64_t t0 = warp_sum61(lane < (uint32_t)FT / 32 ? cx.red[lane * 4] : 0); if (lane == 0) cx.acc[0] = t0; }
         grid_allreduce(cx, a, 1, false);
         if (tid == 0) cx.claim = cx.acc[0];
     }
 
+    VC_TR(11);
     for (int ph = 0; ph < 2; ph++) {
         const uint32_t mode = Lp.mode[ph], K = Lp.K[ph], blo = cp.blo[ph], nbk = cp.nb[ph];
         uint64_t *rr = ph == 0 ? cx.r1 : cx.r2;
@@ -107,6 +108,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             __syncthreads();                     // tables free again before level 1 of phase 2 is built
         }
         uint64_t r_prev = 0;
+        VC_TR(12);
         for (uint32_t j = 0; j < s; j++) {
             bool fence = false;
             const uint64_t *tab = Vb;            // level j as the gates see it (SLICE), or level j-1 (GLOBAL)
@@ -158,7 +160,9 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 }
                 fence = true;
             }
+            VC_TR(13);
             __syncthreads();                     // level j ready in shared memory
+            VC_TR(14);
             // ---- a4 (+ the pending a6 weight update): every gate of this CTA
             if (warp < nw) {
                 const uint64_t omr = fp61::sub(1, r_prev);
@@ -208,7 +212,9 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             }
             // ---- a5 + a6: grid reduction of the three round values, then the challenge
             uint64_t *rslot = rr + j;
+            VC_TR(15);
             round_allreduce(cx, a, nw, fence, tr, rslot, seed, ctr);
+            VC_TR(16);
             ctr++;
             tr += 3;
             r_prev = *rslot;
@@ -228,14 +234,18 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
         }
     }
     if (tid == 0) cx.ctr = ctr;
+    if (b == 0 && warp == 2) transcript_flush(cx, a);       // the last round's message
     __syncthreads();
+    VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
     if (s > 1) {
         line_partials(Vb, s, cx, bufX, b, G, tid, FT);
         grid_allreduce(cx, a, s - 1, false);
     }
+    VC_TR(18);
     line_finish(s, cx, invfact, tr, b == 0, tid);
     __syncthreads();
+    VC_TR(19);
 }
 
 }  // namespace vc
