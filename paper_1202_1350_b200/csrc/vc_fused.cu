@@ -11,7 +11,8 @@ namespace vc {
 __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     extern __shared__ __align__(16) uint8_t smem[];
     FusedCtx &cx = *reinterpret_cast<FusedCtx *>(smem);
-    uint64_t *invfact = reinterpret_cast<uint64_t *>(smem + sizeof(FusedCtx));      // 1/k!, k <= MAX_VARS
+    uint64_t *invfact = reinterpret_cast<uint64_t *>(smem + F_INVFACT_OFF);        // 1/k!, k <= MAX_VARS
+    uint32_t *pas = reinterpret_cast<uint32_t *>(smem + F_PASCAL_OFF);             // C(n,k), n,k < 32
     uint8_t *dyn = smem + F_FIXED_BYTES;
     const uint32_t tid = threadIdx.x;
     // ---- load (or start) the proof state
@@ -24,6 +25,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (tid == 0) { cx.seed = a.seed; cx.ctr = a.st->ctr; cx.claim = a.st->claim; }
     }
     if (tid <= MAX_VARS) invfact[tid] = a.st->invfact[tid];
+    build_pascal(pas, tid);
     if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; cx.pad = 0; cx.pend_tr = nullptr; cx.pend_slot = 0; }
     __syncthreads();
     uint64_t *tr = a.tr;
@@ -33,7 +35,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
         VC_TR(100 + layer);
         if (a.L[layer].kind == 0) {
-            if (blockIdx.x == 0) small_layer(a, cx, invfact, dyn, layer, tr);
+            if (blockIdx.x == 0) small_layer(a, cx, invfact, pas, dyn, layer, tr);
             handoff = true;
         } else {
             if (handoff) {
@@ -49,8 +51,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                 __syncthreads();
                 handoff = false;
             }
-            if (a.L[layer].resident) wide_layer<true>(a, cx, invfact, dyn, layer, tr);
-            else wide_layer<false>(a, cx, invfact, dyn, layer, tr);
+            wide_layer(a, cx, invfact, pas, dyn, layer, tr);
         }
         tr += 7 * (size_t)s + 1;
     }
@@ -86,7 +87,9 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
     const uint64_t n = 1ull << si;
     lp.log_n = si;
     lp.kind = (si <= (uint32_t)F_SMALL_N_LOG && s <= (uint32_t)F_SMALL_T_LOG) ? 0 : 1;
-    lp.resident = 0; lp.cap = 0; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
+    lp.has_relay = 0;
+    for (uint8_t t : c->h_type[i]) if (t == VC_RELAY) { lp.has_relay = 1; break; }
+    lp.resident = 0; lp.cap = 0; lp.gthr = FT; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
     lp.xw = lp.yw = 0; lp.off_tab = lp.off_scr = 0;
     if (lp.kind == 0) { smem_need = std::max(smem_need, F_FIXED_BYTES + F_SMALL_BYTES); return; }
     // gates in units of 32, spread evenly over the CTAs
@@ -108,6 +111,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         }
     }
     const size_t cap = (size_t)((ngmax + FT - 1) / FT) * FT;
+    lp.gthr = FT;                                // one gate per thread first: thin layers are bound by the per-gate latency chain
     const size_t state = cap * 20;
     // fold buffers: odd levels in X, even levels in Y; slices exist for levels 1..K-1
     auto buf_words = [&](int ph, size_t &xw, size_t &yw) {
@@ -116,7 +120,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         if (K >= 2) xw = std::max(xw, (size_t)nbmax[ph] << (K - 1));
         if (K >= 3) yw = std::max(yw, (size_t)nbmax[ph] << (K - 2));
     };
-    const size_t scr_words = 1u << F_EQLOG;
+    const size_t scr_words = (1u << F_EQLOG) + 64;
     bool slice_ok[2];
     for (int ph = 0; ph < 2; ph++) slice_ok[ph] = K <= (uint32_t)F_EQLOG + 1;   // the owner's eq table covers K-1 <= 10 variables
     // try: resident state + slices, then non-resident + slices, then drop the larger slice, ...
@@ -131,9 +135,10 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         size_t X = 1024, Y = 1024;
         for (int ph = 0; ph < 2; ph++) if (use[ph]) { X = std::max(X, xw[ph]); Y = std::max(Y, yw[ph]); }
         X = (X + 1) & ~(size_t)1; Y = (Y + 1) & ~(size_t)1;
-        const size_t tabw = std::max<size_t>(X + Y, std::max<size_t>(4u << F_EQLOG, fused_line_words(s)));
+        const size_t tabw = std::max<size_t>(X + Y, 4u << F_EQLOG);
         const size_t st_bytes = res ? state : 0;
-        const size_t total = F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8;
+        const size_t total = std::max(F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8,
+                                      F_FIXED_BYTES + fused_line_words(s, FT) * 8);   // the line restriction reuses the whole region
         if (total > F_SMEM_MAX) continue;
         lp.resident = res ? 1 : 0;
         lp.cap = (uint32_t)cap;

@@ -44,7 +44,9 @@ struct LayerPlan {
     uint32_t log_n;
     uint32_t kind;                       // 0: single CTA, 1: grid-wide
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
+    uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
     uint32_t cap;                        // state capacity in gates (multiple of FT)
+    uint32_t gthr;                       // threads per CTA that own gates (multiple of 32, <= FT)
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
     uint32_t xw, yw;                     // words of the two fold buffers
@@ -75,8 +77,11 @@ struct FusedCtx {            // block-shared bookkeeping, replicated in every CT
     uint32_t pend_slot, pad2;
 };
 
-// fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS; the rest starts 16-byte aligned
-constexpr size_t F_FIXED_BYTES = (sizeof(FusedCtx) + (MAX_VARS + 1) * 8 + 15) & ~(size_t)15;
+// fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS, then Pascal's triangle C(n,k),
+// n,k < 32 (u32); the rest starts 16-byte aligned
+constexpr size_t F_INVFACT_OFF = sizeof(FusedCtx);
+constexpr size_t F_PASCAL_OFF = (F_INVFACT_OFF + (MAX_VARS + 1) * 8 + 15) & ~(size_t)15;
+constexpr size_t F_FIXED_BYTES = F_PASCAL_OFF + 32 * 32 * 4;
 
 // Optional fine-grained trace (compile with -DVC_TRACE): CTA 0 / thread 0 appends (code << 48 | SM clock) after the
 // d+1 layer stamps; read back with vc_debug_layer_stamps' buffer via vc_debug_trace.  Off in the product build.
@@ -124,7 +129,7 @@ __device__ __forceinline__ uint64_t warp_sum61(uint64_t v) {
 }
 
 // eq(u, x[k0..k1)) for one index u by direct product, two interleaved chains (no table, no barrier)
-__device__ __forceinline__ uint64_t eq_direct(uint32_t u, const uint64_t *x, uint32_t k0, uint32_t k1) {
+__device__ __noinline__ uint64_t eq_direct(uint32_t u, const uint64_t *x, uint32_t k0, uint32_t k1) {
     uint64_t e0 = 1, e1 = 1;
     uint32_t k = k0;
     for (; k + 1 < k1; k += 2) {
@@ -148,13 +153,36 @@ struct EqTab {
         return e;
     }
 };
-__device__ __forceinline__ EqTab build_eq_tab(uint64_t *lo, uint64_t *hi, const uint64_t *x, uint32_t nv, uint32_t t,
-                                              uint32_t nthr) {
+// eq table over nv <= 10 variables as the outer product of two tables of <= 5 variables each (built by direct
+// product in tmp[0..64)): one multiply per entry instead of nv.  Contains one block barrier; caller syncs afterwards.
+__device__ __noinline__ void build_eq10(uint64_t *out, uint64_t *tmp, const uint64_t *x, uint32_t k0, uint32_t nv,
+                                           uint32_t t, uint32_t nthr) {
+    const uint32_t na = nv < 5 ? nv : 5, nb = nv - na;
+    if (t < 64) {
+        const uint32_t which = t >> 5, u = t & 31;
+        if (which == 0) { if (u < (1u << na)) tmp[u] = eq_direct(u, x, k0, k0 + na); }
+        else if (u < (1u << nb)) tmp[32 + u] = eq_direct(u, x, k0 + na, k0 + nv);
+    }
+    __syncthreads();
+    for (uint32_t u = t; u < (1u << nv); u += nthr) out[u] = fp61::mul(tmp[u & ((1u << na) - 1)], tmp[32 + (u >> na)]);
+}
+// caller provides the barrier afterwards; tmp: 128 words of scratch
+__device__ __noinline__ EqTab build_eq_tab(uint64_t *lo, uint64_t *hi, uint64_t *tmp, const uint64_t *x, uint32_t nv,
+                                              uint32_t t, uint32_t nthr) {
     const uint32_t cl = nv < F_EQLOG ? nv : F_EQLOG;
     const uint32_t ch = nv < 2 * F_EQLOG ? nv : 2 * F_EQLOG;
-    for (uint32_t u = t; u < (1u << cl); u += nthr) lo[u] = eq_direct(u, x, 0, cl);
-    if (ch > cl)
-        for (uint32_t u = t; u < (1u << (ch - cl)); u += nthr) hi[u] = eq_direct(u, x, cl, ch);
+    // both halves share the barrier: the 5-variable tables of the high half are built in tmp[64..128)
+    const uint32_t na = cl < 5 ? cl : 5, nb = cl - na, hv = ch - cl, ha = hv < 5 ? hv : 5, hb = hv - ha;
+    if (t < 128) {
+        const uint32_t which = t >> 5, u = t & 31;
+        if (which == 0) { if (u < (1u << na)) tmp[u] = eq_direct(u, x, 0, na); }
+        else if (which == 1) { if (u < (1u << nb)) tmp[32 + u] = eq_direct(u, x, na, cl); }
+        else if (which == 2) { if (u < (1u << ha)) tmp[64 + u] = eq_direct(u, x, cl, cl + ha); }
+        else if (u < (1u << hb)) tmp[96 + u] = eq_direct(u, x, cl + ha, ch);
+    }
+    __syncthreads();
+    for (uint32_t u = t; u < (1u << cl); u += nthr) lo[u] = fp61::mul(tmp[u & ((1u << na) - 1)], tmp[32 + (u >> na)]);
+    if (hv) for (uint32_t u = t; u < (1u << hv); u += nthr) hi[u] = fp61::mul(tmp[64 + (u & ((1u << ha) - 1))], tmp[96 + (u >> ha)]);
     EqTab e; e.lo = lo; e.hi = hi; e.x = x; e.nv = nv;
     return e;
 }
@@ -163,7 +191,7 @@ __device__ __forceinline__ EqTab build_eq_tab(uint64_t *lo, uint64_t *hi, const 
 // Every CTA adds (low 32 bits | 1<<48) and (high bits | 1<<48) into the slot of this epoch; a word is complete when
 // its count field equals the number of CTAs.  Totals land in cx.acc[k] of every CTA.  With fence = true all global
 // writes made by this CTA before the call are visible to every CTA after it.
-__device__ __forceinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t K, bool fence) {
+__device__ __noinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t K, bool fence) {
     const uint32_t tid = threadIdx.x;
     __syncthreads();
     const uint32_t ep = cx.epoch;
@@ -232,12 +260,14 @@ __device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     const uint32_t ep = cx.epoch;        // last written before the trailing barrier of the previous rendezvous
     __syncthreads();
+    VC_TR(31);
     if (tid < 32) {
         unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
         const uint64_t t0 = warp_sum61(lane < nw ? cx.red[lane * 4 + 0] : 0);
         const uint64_t t1 = warp_sum61(lane < nw ? cx.red[lane * 4 + 1] : 0);
         const uint64_t t2 = warp_sum61(lane < nw ? cx.red[lane * 4 + 2] : 0);
         const uint64_t r = fp61::draw(seed, ctr);
+        VC_TR(32);
         if (lane < 6) {
             const uint64_t v = lane < 2 ? t0 : (lane < 4 ? t1 : t2);
             const uint64_t part = ((lane & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE;
@@ -251,6 +281,7 @@ __device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a
                 red_add(slot + lane, part);
             }
         }
+        VC_TR(33);
         if (lane == 0) { cx.epoch = ep + 1; *rslot = r; }
     } else if (blockIdx.x == 0) {
         if (tid >= 64 && tid < 96) {     // transcript of the previous round, then remember this one

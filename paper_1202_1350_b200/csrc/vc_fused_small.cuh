@@ -41,7 +41,7 @@ __device__ __forceinline__ void gate_fin(const acc128 &X, const acc128 &X1, cons
     g[2] = fp61::sub(fp61::add(fp61::dbl(y1), y1), y);
 }
 
-__device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, uint8_t *dyn,
+__device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas, uint8_t *dyn,
                                             uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t si = a.L[layer].log_n, s = a.L[layer + 1].log_n;
@@ -123,7 +123,7 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
         }
         if (tid == 0) cx.ctr = ctr;
         VC_TR(6);
-        if (s > 1) line_partials(Vs, s, cx, scratch, 0, 1, tid, nthr);   // a7 (its first barrier publishes cx.ctr)
+        if (s > 1) line_partials(Vs, s, cx, pas, scratch, 0, 1, tid, nthr);   // a7 (its first barrier publishes cx.ctr)
         else bar_n(nthr);
         VC_TR(7);
         line_finish(s, cx, invfact, tr, true, tid);
@@ -132,6 +132,6 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
     __syncthreads();
 }
 
-constexpr size_t F_SMALL_BYTES = (F_SMALL_WORDS + 11 * 12 + 3 * 11 * 32) * 8;
+constexpr size_t F_SMALL_BYTES = (F_SMALL_WORDS + 13 * 12 + 2 + 512 * 13 + 256 * 13 + 2 + 64) * 8;   // + line scratch, s <= 12
 
 }  // namespace vc

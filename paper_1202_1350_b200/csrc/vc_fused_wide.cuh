@@ -11,6 +11,8 @@
 //   F_MODE_GLOBAL: every level is materialised in global memory by the whole grid and the gates fold level j-1 on the
 //                  fly (two extra multiplies per gate-round); used when a CTA's slice would not fit.
 #pragma once
+#include <type_traits>
+
 #include "vc_fused.cuh"
 #include "vc_fused_line.cuh"
 #include "vc_fused_small.cuh"
@@ -18,12 +20,13 @@
 namespace vc {
 
 // level K-1 of the fold table, entries [e0, e1): T[e] = sum_v eq(v, rr[0..K-1)) V[e 2^(K-1) + v].  One warp per entry.
-__device__ __forceinline__ void publish_level(const uint64_t *__restrict__ Vb, const uint64_t *rr, uint32_t km1, uint32_t e0,
+__device__ __noinline__ void publish_level(const uint64_t *__restrict__ Vb, const uint64_t *rr, uint32_t km1, uint32_t e0,
                                               uint32_t e1, uint64_t *eqt, uint64_t *Tg) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     __syncthreads();                                             // rr[km1-1] (written by the last rendezvous) is visible
-    for (uint32_t v = tid; v < (1u << km1); v += FT) eqt[v] = eq_direct(v, rr, 0, km1);
+    build_eq10(eqt + 64, eqt, rr, 0, km1, tid, FT);              // eqt[0..64): the two 5-variable factors
     __syncthreads();
+    eqt += 64;
     for (uint32_t e = e0 + warp; e < e1; e += FT / 32) {
         const uint64_t *src = Vb + ((size_t)e << km1);
         acc128 A; A.clear();
@@ -37,19 +40,36 @@ __device__ __forceinline__ void publish_level(const uint64_t *__restrict__ Vb, c
     }
 }
 
-template <bool RES>
-__device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, uint8_t *dyn,
+// One resident gate against a shared-memory (or level-0 global) table: pending weight update, then the two products.
+// cP = c + p is what the state holds (any representative of c works as an addend; this one saves the "+ p").
+struct GateIn { uint64_t W, cP; uint32_t idx; };
+__device__ __forceinline__ void gate_apply(GateIn &gi, const ulonglong2 pr, uint32_t j, bool upd, uint64_t r_prev, uint64_t omr,
+                                           bool has_ign, acc128 &X, acc128 &X1, acc128 &Y, acc128 &Y1) {
+    if (upd) gi.W = fp61::mul(gi.W, ((gi.idx >> (j - 1)) & 1u) ? r_prev : omr);
+    uint64_t lo = pr.x, hi = pr.y;
+    if (has_ign && (gi.idx >> 31)) { lo = 0; hi = 0; }
+    const uint32_t bit = (gi.idx >> j) & 1u;
+    const uint64_t mb = (bit ? hi : lo) + gi.cP;                 // < 2^61 + 2^62
+    const uint64_t m2 = 2 * hi + gi.cP - lo;                     // 2 hi - lo + c + p  in (0, 2^63.4)
+    fp61::mac2(X.lo, X.hi, X1.lo, X1.hi, gi.W, mb, bit);
+    fp61::mac2(Y.lo, Y.hi, Y1.lo, Y1.hi, gi.W, m2, bit);
+}
+
+__device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas, uint8_t *dyn,
                                            uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x, b = blockIdx.x;
     const LayerPlan &Lp = a.L[layer];
     const uint32_t si = Lp.log_n, s = a.L[layer + 1].log_n;
+    const bool res = Lp.resident != 0, has_ign = Lp.has_relay != 0;
     const uint64_t *__restrict__ Vb = a.L[layer + 1].V;
     const uint8_t *__restrict__ gtype = Lp.type;
     const uint32_t *__restrict__ gin1 = Lp.in1, *__restrict__ gin2 = Lp.in2;
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;
     const uint32_t nk = (ng + FT - 1) / FT;
-    const uint32_t nw = ng >= (uint32_t)FT ? (uint32_t)FT / 32 : (ng + 31) / 32;   // warps that own gates
+    const uint32_t GT = Lp.gthr;                 // threads that own gates (a thin layer gives each of few threads several)
+    const uint32_t nmine = (tid < GT && tid < ng) ? (ng - tid + GT - 1) / GT : 0;   // this thread's gates: l = k GT + tid
+    const uint32_t nw = ng >= GT ? GT / 32 : (ng + 31) / 32;             // warps that own gates
     const uint32_t cap = Lp.cap;
     uint64_t *sW = reinterpret_cast<uint64_t *>(dyn);
     uint64_t *sC = sW + cap;
@@ -61,20 +81,27 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     // ---- a3: beta(z, g) through a two-level eq table (built in the fold buffers, which are idle until level 1)
     __syncthreads();
     uint32_t ctr = (uint32_t)cx.ctr;
-    const EqTab eb = build_eq_tab(bufX, bufX + (1u << F_EQLOG), cx.z, si, tid, FT);
+    const EqTab eb = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);
     __syncthreads();
     uint64_t claim_part = 0;
-    for (uint32_t k = 0; k < nk; k++) {
-        const uint32_t l = k * FT + tid;
-        if (l >= ng) break;
-        const uint32_t g = g0 + l;
-        const uint64_t P = eb.eq_of(g);
-        const uint32_t i1 = gin1[g], i2 = gin2[g], t = gtype[g];
-        uint64_t W, c; uint32_t ign;
-        gate_state(1, t, P, Vb[i2], W, c, ign);
-        if (RES) { sW[l] = W; sC[l] = c; sI[l] = i1; } else { a.P[g] = W; a.C[g] = c; }
-        if (layer == 0) claim_part = fp61::add(claim_part, fp61::mul(P, Lp.V[g]));
-    }
+    auto setup1 = [&](auto resident) {
+#pragma unroll 2
+        for (uint32_t k = 0; k < nk; k++) {
+            const uint32_t l = k * FT + tid;
+            const bool valid = l < ng;
+            const uint32_t g = valid ? g0 + l : g0;
+            const uint32_t i1 = __ldg(gin1 + g), i2 = __ldg(gin2 + g), t = __ldg(gtype + g);
+            const uint64_t other = __ldg(Vb + i2);
+            const uint64_t P = eb.eq_of(g);
+            uint64_t W, c; uint32_t ign;
+            gate_state(1, t, P, other, W, c, ign);
+            if (valid) {
+                if (decltype(resident)::value) { sW[l] = W; sC[l] = c + fp61::P; sI[l] = i1; } else { a.P[g] = W; a.C[g] = c + fp61::P; }
+                if (layer == 0) claim_part = fp61::add(claim_part, fp61::mul(P, __ldg(Lp.V + g)));
+            }
+        }
+    };
+    if (res) setup1(std::true_type{}); else setup1(std::false_type{});
     if (layer == 0) {                            // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
         claim_part = warp_sum61(claim_part);
         if (lane == 0) cx.red[warp * 4] = claim_part;
@@ -92,19 +119,26 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             // ---- phase switch: plain weight P = beta(z,g) eq(in1[g], r1), then the phase-2 state
             __syncthreads();                     // v1, r1[s-1] visible; phase-1 tables dead
             const uint64_t v1 = cx.v1;
-            const EqTab e0 = build_eq_tab(bufX, bufX + (1u << F_EQLOG), cx.z, si, tid, FT);
-            const EqTab e1 = build_eq_tab(bufX + (2u << F_EQLOG), bufX + (3u << F_EQLOG), cx.r1, s, tid, FT);
+            const EqTab e0 = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);
+            const EqTab e1 = build_eq_tab(bufX + (2u << F_EQLOG), bufX + (3u << F_EQLOG), scr + 128, cx.r1, s, tid, FT);
             __syncthreads();
-            for (uint32_t k = 0; k < nk; k++) {
-                const uint32_t l = k * FT + tid;
-                if (l >= ng) break;
-                const uint32_t g = g0 + l;
-                const uint32_t i1 = gin1[g], i2 = gin2[g], t = gtype[g];
-                const uint64_t P = fp61::mul(e0.eq_of(g), e1.eq_of(i1));
-                uint64_t W, c; uint32_t ign;
-                gate_state(2, t, P, v1, W, c, ign);
-                if (RES) { sW[l] = W; sC[l] = c; sI[l] = i2 | (ign << 31); } else { a.P[g] = W; a.C[g] = c; }
-            }
+            auto setup2 = [&](auto resident) {
+#pragma unroll 2
+                for (uint32_t k = 0; k < nk; k++) {
+                    const uint32_t l = k * FT + tid;
+                    const bool valid = l < ng;
+                    const uint32_t g = valid ? g0 + l : g0;
+                    const uint32_t i1 = __ldg(gin1 + g), i2 = __ldg(gin2 + g), t = __ldg(gtype + g);
+                    const uint64_t P = fp61::mul(e0.eq_of(g), e1.eq_of(i1));
+                    uint64_t W, c; uint32_t ign;
+                    gate_state(2, t, P, v1, W, c, ign);
+                    if (valid) {
+                        if (decltype(resident)::value) { sW[l] = W; sC[l] = c + fp61::P; sI[l] = i2 | (ign << 31); }
+                        else { a.P[g] = W; a.C[g] = c + fp61::P; }
+                    }
+                }
+            };
+            if (res) setup2(std::true_type{}); else setup2(std::false_type{});
             __syncthreads();                     // tables free again before level 1 of phase 2 is built
         }
         uint64_t r_prev = 0;
@@ -121,6 +155,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         const uint32_t cnt = nbk << (K - j);
                         if (j == 1) {
                             const uint64_t *src = Vb + ((size_t)blo << K);
+#pragma unroll 4
                             for (uint32_t v = tid; v < cnt; v += FT) {
                                 const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)v);
                                 dst[v] = fold2(p.x, p.y, r_prev);
@@ -166,44 +201,73 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             // ---- a4 (+ the pending a6 weight update): every gate of this CTA
             if (warp < nw) {
                 const uint64_t omr = fp61::sub(1, r_prev);
+                const bool upd = j >= 1;
                 acc128 X, X1, Y, Y1; X.clear(); X1.clear(); Y.clear(); Y1.clear();
                 uint64_t gs[3] = {0, 0, 0};
-                for (uint32_t k = 0; k < nk; k++) {
-                    const uint32_t l = k * FT + tid;
-                    if (l >= ng) break;
-                    uint64_t W, c; uint32_t idx;
-                    if (RES) { W = sW[l]; c = sC[l]; idx = sI[l]; }
-                    else {
-                        const uint32_t g = g0 + l;
-                        W = a.P[g]; c = a.C[g];
-                        idx = ph == 0 ? gin1[g] : (gin2[g] | ((gtype[g] == VC_RELAY ? 1u : 0u) << 31));
-                    }
-                    if (j >= 1) {
-                        W = fp61::mul(W, ((idx >> (j - 1)) & 1u) ? r_prev : omr);
-                        if (RES) sW[l] = W; else a.P[g0 + l] = W;
-                    }
-                    const uint32_t bit = (idx >> j) & 1u, u = (idx & F_IDX_MASK) >> (j + 1);
-                    uint64_t lo, hi;
-                    if (mode == F_MODE_SLICE || j == 0) {
-                        const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(tab + (2 * (size_t)u - base));
-                        lo = p.x; hi = p.y;
-                    } else {                     // fold level j-1 on the fly with r_{j-1}
-                        const ulonglong2 p0 = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 4 * (size_t)u));
-                        const ulonglong2 p1 = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 4 * (size_t)u + 2));
-                        lo = fold2(p0.x, p0.y, r_prev); hi = fold2(p1.x, p1.y, r_prev);
-                    }
-                    if (idx >> 31) { lo = 0; hi = 0; }
-                    gate_mac(W, c, bit, lo, hi, X, X1, Y, Y1);
-                    if ((k & 7) == 7) {          // 8 products per accumulator at most
-                        uint64_t g3[3];
-                        gate_fin(X, X1, Y, Y1, g3);
+                if (res && mode == F_MODE_SLICE) {
+                    // hot loop: state and table in shared memory (level 0: L2), two gates in flight per thread
+                    const uint64_t *tb = tab - base;
+                    const uint32_t sh = j + 1;
+                    uint32_t k = 0;
+                    for (; k + 2 <= nmine; k += 2) {
+                        const uint32_t l0 = k * GT + tid, l1 = l0 + GT;
+                        GateIn A, B;
+                        A.W = sW[l0]; A.cP = sC[l0]; A.idx = sI[l0];
+                        B.W = sW[l1]; B.cP = sC[l1]; B.idx = sI[l1];
+                        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((A.idx & F_IDX_MASK) >> sh));
+                        const ulonglong2 pb = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((B.idx & F_IDX_MASK) >> sh));
+                        gate_apply(A, pa, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
+                        gate_apply(B, pb, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
+                        if (upd) { sW[l0] = A.W; sW[l1] = B.W; }
+                        if ((k & 6) == 6) {      // 8 products per accumulator at most
+                            uint64_t g3[3];
+                            gate_fin(X, X1, Y, Y1, g3);
 #pragma unroll
-                        for (int q = 0; q < 3; q++) gs[q] = fp61::add(gs[q], g3[q]);
-                        X.clear(); X1.clear(); Y.clear(); Y1.clear();
+                            for (int q = 0; q < 3; q++) gs[q] = fp61::add(gs[q], g3[q]);
+                            X.clear(); X1.clear(); Y.clear(); Y1.clear();
+                        }
+                    }
+                    if (k < nmine) {
+                        const uint32_t l0 = k * GT + tid;
+                        GateIn A;
+                        A.W = sW[l0]; A.cP = sC[l0]; A.idx = sI[l0];
+                        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((A.idx & F_IDX_MASK) >> sh));
+                        gate_apply(A, pa, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
+                        if (upd) sW[l0] = A.W;
+                    }
+                } else {
+                    for (uint32_t k = 0; k < nmine; k++) {
+                        const uint32_t l = k * GT + tid, g = g0 + l;
+                        GateIn A;
+                        if (res) { A.W = sW[l]; A.cP = sC[l]; A.idx = sI[l]; }
+                        else {
+                            A.W = a.P[g]; A.cP = a.C[g];
+                            A.idx = ph == 0 ? gin1[g] : (gin2[g] | ((gtype[g] == VC_RELAY ? 1u : 0u) << 31));
+                        }
+                        const uint32_t u = (A.idx & F_IDX_MASK) >> (j + 1);
+                        ulonglong2 pr;
+                        if (mode == F_MODE_SLICE || j == 0) {
+                            pr = *reinterpret_cast<const ulonglong2 *>(tab + (2 * (size_t)u - base));
+                        } else {                 // fold level j-1 on the fly with r_{j-1}
+                            const ulonglong2 p0 = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 4 * (size_t)u));
+                            const ulonglong2 p1 = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 4 * (size_t)u + 2));
+                            pr.x = fold2(p0.x, p0.y, r_prev); pr.y = fold2(p1.x, p1.y, r_prev);
+                        }
+                        gate_apply(A, pr, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
+                        if (upd) { if (res) sW[l] = A.W; else a.P[g] = A.W; }
+                        if ((k & 7) == 7) {
+                            uint64_t g3[3];
+                            gate_fin(X, X1, Y, Y1, g3);
+#pragma unroll
+                            for (int q = 0; q < 3; q++) gs[q] = fp61::add(gs[q], g3[q]);
+                            X.clear(); X1.clear(); Y.clear(); Y1.clear();
+                        }
                     }
                 }
+                VC_TR(21);
                 uint64_t g3[3];
                 gate_fin(X, X1, Y, Y1, g3);
+                VC_TR(22);
 #pragma unroll
                 for (int q = 0; q < 3; q++) {
                     const uint64_t v = warp_sum61(fp61::add(gs[q], g3[q]));
@@ -239,7 +303,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
     if (s > 1) {
-        line_partials(Vb, s, cx, bufX, b, G, tid, FT);
+        line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, FT);
         grid_allreduce(cx, a, s - 1, false);
     }
     VC_TR(18);
