@@ -4,6 +4,7 @@
 
 #include "vc_circuit.hpp"
 #include "vc_fused_small.cuh"
+#include "vc_fused_thin.cuh"
 #include "vc_fused_wide.cuh"
 
 namespace vc {
@@ -51,7 +52,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                 __syncthreads();
                 handoff = false;
             }
-            wide_layer(a, cx, invfact, pas, dyn, layer, tr);
+            if (a.L[layer].thin) thin_layer(a, cx, invfact, pas, dyn, layer, tr);
+            else wide_layer(a, cx, invfact, pas, dyn, layer, tr);
         }
         tr += 7 * (size_t)s + 1;
     }
@@ -89,8 +91,8 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
     lp.kind = (si <= (uint32_t)F_SMALL_N_LOG && s <= (uint32_t)F_SMALL_T_LOG) ? 0 : 1;
     lp.has_relay = 0;
     for (uint8_t t : c->h_type[i]) if (t == VC_RELAY) { lp.has_relay = 1; break; }
-    lp.resident = 0; lp.cap = 0; lp.gthr = FT; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
-    lp.xw = lp.yw = 0; lp.off_tab = lp.off_scr = 0;
+    lp.thin = 0; lp.resident = 0; lp.cap = 0; lp.gthr = FT; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
+    lp.xw = lp.yw = 0; lp.off_tab = lp.off_scr = lp.off_commit = 0;
     if (lp.kind == 0) { smem_need = std::max(smem_need, F_FIXED_BYTES + F_SMALL_BYTES); return; }
     // gates in units of 32, spread evenly over the CTAs
     const uint64_t U = (n + 31) / 32;
@@ -123,6 +125,24 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
     const size_t scr_words = (1u << F_EQLOG) + 64;
     bool slice_ok[2];
     for (int ph = 0; ph < 2; ph++) slice_ok[ph] = K <= (uint32_t)F_EQLOG + 1;   // the owner's eq table covers K-1 <= 10 variables
+    if (ngmax <= F_WORKERS && slice_ok[0] && slice_ok[1]) {     // thin layer: gate in registers, commit buffers instead of state
+        size_t xw[2], yw[2];
+        buf_words(0, xw[0], yw[0]); buf_words(1, xw[1], yw[1]);
+        size_t X = std::max<size_t>(1024, std::max(xw[0], xw[1])), Y = std::max<size_t>(1024, std::max(yw[0], yw[1]));
+        X = (X + 1) & ~(size_t)1; Y = (Y + 1) & ~(size_t)1;
+        const size_t tabw = std::max<size_t>(X + Y, 4u << F_EQLOG);
+        const size_t total = std::max(F_FIXED_BYTES + F_THIN_COMMIT_BYTES + tabw * 8 + scr_words * 8,
+                                      F_FIXED_BYTES + fused_line_words(s, FT) * 8);
+        if (total <= F_SMEM_MAX) {
+            lp.thin = 1; lp.cap = (uint32_t)cap;
+            for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = F_MODE_SLICE; lp.K[ph] = K; }
+            lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
+            lp.off_tab = (uint32_t)F_THIN_COMMIT_BYTES;
+            lp.off_scr = (uint32_t)(F_THIN_COMMIT_BYTES + tabw * 8);
+            smem_need = std::max(smem_need, total);
+            return;
+        }
+    }
     // try: resident state + slices, then non-resident + slices, then drop the larger slice, ...
     for (int attempt = 0; attempt < 6; attempt++) {
         const bool res = attempt < 3;
@@ -137,7 +157,8 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         X = (X + 1) & ~(size_t)1; Y = (Y + 1) & ~(size_t)1;
         const size_t tabw = std::max<size_t>(X + Y, 4u << F_EQLOG);
         const size_t st_bytes = res ? state : 0;
-        const size_t total = std::max(F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8,
+        const size_t commit_bytes = (size_t)F_WORKERS * 32;
+        const size_t total = std::max(F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8 + commit_bytes,
                                       F_FIXED_BYTES + fused_line_words(s, FT) * 8);   // the line restriction reuses the whole region
         if (total > F_SMEM_MAX) continue;
         lp.resident = res ? 1 : 0;
@@ -146,6 +167,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
         lp.off_tab = (uint32_t)st_bytes;
         lp.off_scr = (uint32_t)(st_bytes + tabw * 8);
+        lp.off_commit = (uint32_t)(st_bytes + tabw * 8 + scr_words * 8);
         smem_need = std::max(smem_need, total);
         return;
     }

@@ -25,7 +25,7 @@ constexpr int F_EQLOG = 10;              // eq tables are built in halves of at 
 constexpr int F_SMALL_N_LOG = 9;         // single-CTA path: gates <= 2^9 (one per thread) ...
 constexpr int F_SMALL_T_LOG = 12;        // ... and table <= 2^12 words
 constexpr int F_SLOT_WORDS = 128;        // one rendezvous slot: up to 64 values x (lo,hi)
-constexpr int F_RING = 4;
+constexpr int F_RING = 8;                // slots are recycled two epochs ahead and converted up to two epochs late
 constexpr uint64_t F_CNT_ONE = 1ull << 48;
 constexpr uint64_t F_VAL_MASK = F_CNT_ONE - 1;
 constexpr uint32_t F_IDX_MASK = 0x3fffffffu;   // indices are < 2^30; bit 31 of a packed index = "x ignored" (RELAY, phase 2)
@@ -43,6 +43,7 @@ struct LayerPlan {
     const CtaPlan *cta;                  // gridDim entries (wide layers), else null
     uint32_t log_n;
     uint32_t kind;                       // 0: single CTA, 1: grid-wide
+    uint32_t thin;                       // 1: at most one gate per worker thread: vc_fused_thin.cuh
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
     uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
     uint32_t cap;                        // state capacity in gates (multiple of FT)
@@ -50,7 +51,7 @@ struct LayerPlan {
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
     uint32_t xw, yw;                     // words of the two fold buffers
-    uint32_t off_tab, off_scr;           // byte offsets in dynamic shared memory (after the state)
+    uint32_t off_tab, off_scr, off_commit;   // byte offsets in dynamic shared memory (after the state)
 };
 
 struct FusedArgs {
@@ -293,6 +294,73 @@ __device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a
         }
     }
     __syncthreads();
+}
+
+// ---- warp-specialised rounds (vc_fused_thin.cuh, vc_fused_wide.cuh): warps 0..14 work, warp 15 reduces.
+constexpr uint32_t F_WORKERS = FT - 32;          // threads of warps 0..14
+__device__ __forceinline__ void bar_workers() { asm volatile("bar.sync 2, %0;" ::"r"(F_WORKERS) : "memory"); }
+// (hi:lo) += v if pred
+__device__ __forceinline__ void add_c(uint64_t &lo, uint32_t &hi, uint64_t v, uint32_t pred) {
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p add.cc.u64 %0, %0, %2;\n\t@p addc.u32 %1, %1, 0;\n\t}"
+        : "+l"(lo), "+r"(hi) : "l"(v), "r"(pred));
+}
+// round slot: word 0 = count only (the rendezvous), words 1..6 = (low 32 | count), (high | count) of G0, G1, G2
+__device__ __forceinline__ void round_slot_to_transcript(const unsigned long long *slot, uint64_t *tr, uint32_t lane) {
+    uint64_t got = 0;
+    if (lane >= 1 && lane < 7) {
+        const uint64_t want = (uint64_t)gridDim.x;
+        unsigned long long w;
+        while (((w = ld_relaxed(slot + lane)) >> 48) != want) { }
+        got = w & F_VAL_MASK;
+    }
+    const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
+    if (lane >= 1 && lane < 7 && (lane & 1)) tr[(lane - 1) >> 1] = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
+}
+// warp 0, after the commit barrier: the rendezvous on the count word; the challenge is handed out afterwards
+__device__ __forceinline__ void round_rendezvous(const FusedArgs &a, uint32_t ep, bool fence, uint64_t *rslot, uint64_t seed,
+                                                 uint32_t ctr) {
+    const uint64_t r = fp61::draw(seed, ctr);
+    if ((threadIdx.x & 31) == 0) {
+        unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
+        if (fence) __threadfence();
+        const uint64_t want = (uint64_t)gridDim.x;
+        if ((atom_add(slot, F_CNT_ONE) >> 48) + 1 != want)
+            while ((ld_relaxed(slot) >> 48) != want) { }
+        if (fence) __threadfence();
+        *rslot = r;
+    }
+}
+// the reducer's bookkeeping in CTA 0: transcript positions of the last two rounds whose slots are not converted yet
+struct RoundPend { uint64_t *tr1, *tr2; uint32_t s1, s2; };
+// warp 15: the CTA totals t0..t2 (all lanes) go to the round's data words; CTA 0 converts the slot of two rounds ago
+// into transcript words and recycles the slot of epoch+2
+__device__ __forceinline__ void reducer_post(const FusedArgs &a, uint32_t ep, uint64_t t0, uint64_t t1, uint64_t t2, uint64_t *tr,
+                                             RoundPend &pd) {
+    const uint32_t lane = threadIdx.x & 31;
+    unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
+    if (lane >= 1 && lane < 7) {
+        const uint32_t k = (lane - 1) >> 1;
+        const uint64_t v = k == 0 ? t0 : (k == 1 ? t1 : t2);
+        red_add(slot + lane, (((lane - 1) & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE);
+    }
+    if (blockIdx.x == 0) {
+        if (pd.tr2) round_slot_to_transcript(a.slots + (size_t)pd.s2 * F_SLOT_WORDS, pd.tr2, lane);
+        pd.tr2 = pd.tr1; pd.s2 = pd.s1; pd.tr1 = tr; pd.s1 = ep % F_RING;
+    }
+    if (blockIdx.x == gridDim.x - 1) {   // slot recycling is the last CTA's job (CTA 0 already has the transcript)
+        unsigned long long *z = a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS;
+#pragma unroll
+        for (int q = 0; q < F_SLOT_WORDS / 32; q++) z[q * 32 + lane] = 0ull;
+        __threadfence();
+    }
+}
+__device__ __forceinline__ void reducer_flush(const FusedArgs &a, RoundPend &pd) {
+    const uint32_t lane = threadIdx.x & 31;
+    if (blockIdx.x == 0) {
+        if (pd.tr2) round_slot_to_transcript(a.slots + (size_t)pd.s2 * F_SLOT_WORDS, pd.tr2, lane);
+        if (pd.tr1) round_slot_to_transcript(a.slots + (size_t)pd.s1 * F_SLOT_WORDS, pd.tr1, lane);
+    }
+    pd.tr1 = pd.tr2 = nullptr;
 }
 
 }  // namespace vc

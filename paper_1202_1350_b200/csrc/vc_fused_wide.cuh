@@ -67,9 +67,9 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;
     const uint32_t nk = (ng + FT - 1) / FT;
-    const uint32_t GT = Lp.gthr;                 // threads that own gates (a thin layer gives each of few threads several)
-    const uint32_t nmine = (tid < GT && tid < ng) ? (ng - tid + GT - 1) / GT : 0;   // this thread's gates: l = k GT + tid
-    const uint32_t nw = ng >= GT ? GT / 32 : (ng + 31) / 32;             // warps that own gates
+    constexpr uint32_t GT = F_WORKERS;           // warps 0..14 own the gates: l = k GT + tid; warp 15 is the reducer
+    const uint32_t nmine = (tid < GT && tid < ng) ? (ng - tid + GT - 1) / GT : 0;
+    ulonglong2 *cbuf = reinterpret_cast<ulonglong2 *>(dyn + Lp.off_commit);       // [GT][2]: X, X1, Y, Y1 sums per worker
     const uint32_t cap = Lp.cap;
     uint64_t *sW = reinterpret_cast<uint64_t *>(dyn);
     uint64_t *sC = sW + cap;
@@ -112,6 +112,10 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     }
 
     VC_TR(11);
+    __syncthreads();
+    uint32_t ep = cx.epoch;
+    RoundPend pd; pd.tr1 = pd.tr2 = nullptr; pd.s1 = pd.s2 = 0;
+    bool first = true;
     for (int ph = 0; ph < 2; ph++) {
         const uint32_t mode = Lp.mode[ph], K = Lp.K[ph], blo = cp.blo[ph], nbk = cp.nb[ph];
         uint64_t *rr = ph == 0 ? cx.r1 : cx.r2;
@@ -156,24 +160,24 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         if (j == 1) {
                             const uint64_t *src = Vb + ((size_t)blo << K);
 #pragma unroll 4
-                            for (uint32_t v = tid; v < cnt; v += FT) {
+                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) {
                                 const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)v);
                                 dst[v] = fold2(p.x, p.y, r_prev);
                             }
                         } else {
-                            for (uint32_t v = tid; v < cnt; v += FT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
+                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
                         }
                         base = blo << (K - j);
                     } else {                     // the whole table: from the published level K-1 (j = K >= 2), from V (j = 1),
                         const uint32_t cnt = 1u << (s - j);                         // else from the previous buffer
                         if (j == 1 || j == K) {
                             const uint64_t *src = j == 1 ? Vb : a.Tg;
-                            for (uint32_t v = tid; v < cnt; v += FT) {
+                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) {
                                 const ulonglong2 p = __ldcg(reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)v));
                                 dst[v] = fold2(p.x, p.y, r_prev);
                             }
                         } else {
-                            for (uint32_t v = tid; v < cnt; v += FT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
+                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
                         }
                     }
                     tab = dst;
@@ -188,7 +192,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 if (j >= 1) {
                     uint64_t *Aout = (j & 1) ? a.T0 : a.T1;                          // level j
                     const uint32_t cnt = 1u << (s - j);
-                    for (uint32_t v = b * FT + tid; v < cnt; v += G * FT) {
+                    if (tid < GT) for (uint32_t v = b * GT + tid; v < cnt; v += G * GT) {
                         const ulonglong2 p = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 2 * (size_t)v));
                         __stcg(Aout + v, fold2(p.x, p.y, r_prev));
                     }
@@ -196,14 +200,14 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 fence = true;
             }
             VC_TR(13);
-            __syncthreads();                     // level j ready in shared memory
+            if (tid < GT) bar_workers();         // level j ready in shared memory (the reducer is still busy with round j-1)
             VC_TR(14);
             // ---- a4 (+ the pending a6 weight update): every gate of this CTA
-            if (warp < nw) {
+            if (tid < GT) {
                 const uint64_t omr = fp61::sub(1, r_prev);
                 const bool upd = j >= 1;
                 acc128 X, X1, Y, Y1; X.clear(); X1.clear(); Y.clear(); Y1.clear();
-                uint64_t gs[3] = {0, 0, 0};
+                uint64_t s4[4] = {0, 0, 0, 0};                 // canonical running sums of X, X1, Y, Y1 (flushed every 8 products)
                 if (res && mode == F_MODE_SLICE) {
                     // hot loop: state and table in shared memory (level 0: L2), two gates in flight per thread
                     const uint64_t *tb = tab - base;
@@ -220,10 +224,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         gate_apply(B, pb, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
                         if (upd) { sW[l0] = A.W; sW[l1] = B.W; }
                         if ((k & 6) == 6) {      // 8 products per accumulator at most
-                            uint64_t g3[3];
-                            gate_fin(X, X1, Y, Y1, g3);
-#pragma unroll
-                            for (int q = 0; q < 3; q++) gs[q] = fp61::add(gs[q], g3[q]);
+                            s4[0] = fp61::add(s4[0], X.value()); s4[1] = fp61::add(s4[1], X1.value());
+                            s4[2] = fp61::add(s4[2], Y.value()); s4[3] = fp61::add(s4[3], Y1.value());
                             X.clear(); X1.clear(); Y.clear(); Y1.clear();
                         }
                     }
@@ -256,32 +258,43 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         gate_apply(A, pr, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
                         if (upd) { if (res) sW[l] = A.W; else a.P[g] = A.W; }
                         if ((k & 7) == 7) {
-                            uint64_t g3[3];
-                            gate_fin(X, X1, Y, Y1, g3);
-#pragma unroll
-                            for (int q = 0; q < 3; q++) gs[q] = fp61::add(gs[q], g3[q]);
+                            s4[0] = fp61::add(s4[0], X.value()); s4[1] = fp61::add(s4[1], X1.value());
+                            s4[2] = fp61::add(s4[2], Y.value()); s4[3] = fp61::add(s4[3], Y1.value());
                             X.clear(); X1.clear(); Y.clear(); Y1.clear();
                         }
                     }
                 }
                 VC_TR(21);
-                uint64_t g3[3];
-                gate_fin(X, X1, Y, Y1, g3);
-                VC_TR(22);
-#pragma unroll
-                for (int q = 0; q < 3; q++) {
-                    const uint64_t v = warp_sum61(fp61::add(gs[q], g3[q]));
-                    if (lane == 0) cx.red[warp * 4 + q] = v;
+                if (!first) asm volatile("bar.sync 3, %0;" ::"r"((uint32_t)FT) : "memory");   // the reducer is done with round j-1's words
+                if (tid < ng) {                  // commit this worker's four sums (any representative < 2^62 will do)
+                    ulonglong2 o0, o1;
+                    o0.x = s4[0] + X.value(); o0.y = s4[1] + X1.value(); o1.x = s4[2] + Y.value(); o1.y = s4[3] + Y1.value();
+                    cbuf[2 * tid] = o0; cbuf[2 * tid + 1] = o1;
                 }
             }
-            // ---- a5 + a6: grid reduction of the three round values, then the challenge
-            uint64_t *rslot = rr + j;
             VC_TR(15);
-            round_allreduce(cx, a, nw, fence, tr, rslot, seed, ctr);
+            __syncthreads();                     // every contribution of this CTA to message j is committed
+            uint64_t *rslot = rr + j;
+            if (warp == 15) {
+                // ---- a5, off the workers' critical path: sum the committed words, add them to the round's data words
+                const uint32_t nc = ng < GT ? ng : GT;
+                uint64_t Sl = 0, S1l = 0, Tl = 0, T1l = 0; uint32_t Sh = 0, S1h = 0, Th = 0, T1h = 0;
+                for (uint32_t i = lane; i < nc; i += 32) {
+                    const ulonglong2 q0 = cbuf[2 * i], q1 = cbuf[2 * i + 1];
+                    add_c(Sl, Sh, q0.x, 1u); add_c(S1l, S1h, q0.y, 1u); add_c(Tl, Th, q1.x, 1u); add_c(T1l, T1h, q1.y, 1u);
+                }
+                if (!(ph == 1 && j + 1 == s)) asm volatile("bar.arrive 3, %0;" ::"r"((uint32_t)FT) : "memory");   // words consumed
+                const uint64_t x = fp61::fold128(Sh, Sl), x1 = fp61::fold128(S1h, S1l), y = fp61::fold128(Th, Tl), y1 = fp61::fold128(T1h, T1l);
+                const uint64_t t0 = warp_sum61(fp61::sub(x, x1)), t1 = warp_sum61(x1);
+                const uint64_t t2 = warp_sum61(fp61::sub(fp61::add(fp61::dbl(y1), y1), y));
+                reducer_post(a, ep, t0, t1, t2, tr, pd);
+            } else {
+                if (warp == 0) round_rendezvous(a, ep, fence, rslot, seed, ctr);   // ---- a6: rendezvous, then the challenge
+                bar_workers();
+            }
             VC_TR(16);
-            ctr++;
-            tr += 3;
-            r_prev = *rslot;
+            ctr++; tr += 3; ep++; first = false;
+            r_prev = *rslot;                     // (the reducer does not use it)
         }
         // ---- V~_{i+1}(r) = the two entries of level s-1 folded with the last challenge
         if (tid == 0) {
@@ -297,8 +310,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             if (ph == 0) cx.v1 = val; else cx.v2 = val;
         }
     }
-    if (tid == 0) cx.ctr = ctr;
-    if (b == 0 && warp == 2) transcript_flush(cx, a);       // the last round's message
+    if (tid == 0) { cx.ctr = ctr; cx.epoch = ep; }
+    if (warp == 15) reducer_flush(a, pd);                   // the last two rounds' messages
     __syncthreads();
     VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
