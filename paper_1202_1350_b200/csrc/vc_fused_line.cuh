@@ -20,6 +20,11 @@ __host__ __device__ inline uint32_t fused_line_tb(uint32_t s, uint32_t nthr) {
     while ((2u << lg) <= nthr) lg++;
     return (sp - 3) < lg ? (sp - 3) : lg;
 }
+// grid-wide layers: blocks of 2^tb threads with tb chosen so that there are at least ~128 blocks to spread over the CTAs
+__host__ __device__ inline uint32_t fused_line_tb_grid(uint32_t s, uint32_t nthr) {
+    const uint32_t sp = s < 3 ? 3 : s, cap = sp > 10 ? sp - 10 : 0, tb = fused_line_tb(s, nthr);
+    return tb < cap ? tb : cap;
+}
 // scratch words: pts[(s+1)*sp (even)] | A[2^tb * P] | B[2^tb * P / 2] | fx[32] | dl[32]
 __host__ __device__ inline size_t fused_line_words(uint32_t s, uint32_t nthr) {
     const size_t sp = s < 3 ? 3 : s, tb = fused_line_tb(s, nthr), P = tb + 4, NB = (size_t)1 << tb;
@@ -40,9 +45,10 @@ __device__ __forceinline__ void build_pascal(uint32_t *pas, uint32_t tid) {
 // cx.acc[t-2] <- sum over this CTA's share (blocks vb0, vb0+vbstride, ...) of eq(u, l(t)) V[u], t = 2..s.
 // Threads tid < nthr take part (nthr a power of two >= 32); they synchronise with bar_n(nthr).  Requires s >= 2.
 __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, FusedCtx &cx, const uint32_t *pas,
-                                              uint64_t *scratch, uint32_t vb0, uint32_t vbstride, uint32_t tid, uint32_t nthr) {
+                                              uint64_t *scratch, uint32_t vb0, uint32_t vbstride, uint32_t tid, uint32_t nthr,
+                                              uint32_t tb) {
     const uint32_t m = s - 1, sp = s < 3 ? 3 : s;
-    const uint32_t tb = fused_line_tb(s, nthr), P = tb + 4, NB = 1u << tb;
+    const uint32_t P = tb + 4, NB = 1u << tb;
     const uint32_t nvb = 1u << (sp - 3 - tb);
     uint64_t *pts = scratch;                                     // pts[t*sp + k] = l(t)_k, t = 0..s; padded variables sit at 0
     uint64_t *A = pts + ((((size_t)s + 1) * sp + 1) & ~(size_t)1);

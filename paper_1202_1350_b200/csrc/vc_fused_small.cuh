@@ -123,7 +123,7 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
         }
         if (tid == 0) cx.ctr = ctr;
         VC_TR(6);
-        if (s > 1) line_partials(Vs, s, cx, pas, scratch, 0, 1, tid, nthr);   // a7 (its first barrier publishes cx.ctr)
+        if (s > 1) line_partials(Vs, s, cx, pas, scratch, 0, 1, tid, nthr, fused_line_tb(s, nthr));   // a7 (its first barrier publishes cx.ctr)
         else bar_n(nthr);
         VC_TR(7);
         line_finish(s, cx, invfact, tr, true, tid);

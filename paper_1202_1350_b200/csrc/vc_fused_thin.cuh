@@ -175,7 +175,8 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
     VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
     if (s > 1) {
-        line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, FT);
+        const uint32_t ltb = fused_line_tb_grid(s, FT), lthr = (1u << ltb) > 32 ? (1u << ltb) : 32;
+        if (tid < lthr) line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, lthr, ltb);
         grid_allreduce(cx, a, s - 1, false);
     }
     VC_TR(18);

@@ -30,13 +30,32 @@ __device__ __noinline__ void publish_level(const uint64_t *__restrict__ Vb, cons
     for (uint32_t e = e0 + warp; e < e1; e += FT / 32) {
         const uint64_t *src = Vb + ((size_t)e << km1);
         acc128 A; A.clear();
-        uint64_t sum = 0; uint32_t it = 0;
-        for (uint32_t v = lane; v < (1u << km1); v += 32) {
-            A.mac(eqt[v], src[v]);
-            if (++it == 32) { sum = fp61::add(sum, A.value()); A.clear(); it = 0; }
+        uint64_t sum = 0;
+        const uint32_t nv = 1u << km1;
+        for (uint32_t v0 = lane; v0 < nv; v0 += 32 * 8) {        // 8 loads in flight per lane, then 8 products
+            uint64_t w[8];
+#pragma unroll
+            for (int q = 0; q < 8; q++) w[q] = v0 + 32 * q < nv ? __ldg(src + v0 + 32 * q) : 0;
+#pragma unroll
+            for (int q = 0; q < 8; q++) if (v0 + 32 * q < nv) A.mac(eqt[v0 + 32 * q], w[q]);
+            sum = fp61::add(sum, A.value()); A.clear();
         }
-        sum = warp_sum61(fp61::add(sum, A.value()));
+        sum = warp_sum61(sum);
         if (lane == 0) __stcg(Tg + e, sum);
+    }
+}
+
+// dst[v] = fold(src[2v], src[2v+1]; r), v < cnt, src in global memory (read-only); 4 loads in flight per thread
+__device__ __noinline__ void fold_level_from_global(uint64_t *dst, const uint64_t *src, uint32_t cnt, uint64_t r, uint32_t t,
+                                                    uint32_t nthr) {
+    for (uint32_t v0 = t; v0 < cnt; v0 += 4 * nthr) {
+        ulonglong2 p[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+            if (v0 + q * nthr < cnt) p[q] = __ldg(reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)(v0 + q * nthr)));
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+            if (v0 + q * nthr < cnt) dst[v0 + q * nthr] = fold2(p[q].x, p[q].y, r);
     }
 }
 
@@ -159,11 +178,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         const uint32_t cnt = nbk << (K - j);
                         if (j == 1) {
                             const uint64_t *src = Vb + ((size_t)blo << K);
-#pragma unroll 4
-                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) {
-                                const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)v);
-                                dst[v] = fold2(p.x, p.y, r_prev);
-                            }
+                            if (tid < GT) fold_level_from_global(dst, src, cnt, r_prev, tid, GT);
                         } else {
                             if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
                         }
@@ -316,7 +331,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
     if (s > 1) {
-        line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, FT);
+        const uint32_t ltb = fused_line_tb_grid(s, FT), lthr = (1u << ltb) > 32 ? (1u << ltb) : 32;
+        if (tid < lthr) line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, lthr, ltb);
         grid_allreduce(cx, a, s - 1, false);
     }
     VC_TR(18);
