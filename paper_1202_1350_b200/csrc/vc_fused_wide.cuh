@@ -74,6 +74,58 @@ __device__ __forceinline__ void gate_apply(GateIn &gi, const ulonglong2 pr, uint
     fp61::mac2(Y.lo, Y.hi, Y1.lo, Y1.hi, gi.W, m2, bit);
 }
 
+// (lo,hi) += a*b
+__device__ __forceinline__ void mac1(acc128 &A, uint64_t pl, uint64_t ph) {
+    asm("add.cc.u64 %0, %0, %2;\n\taddc.u64 %1, %1, %3;" : "+l"(A.lo), "+l"(A.hi) : "l"(pl), "l"(ph));
+}
+// The resident hot loop: this thread's gates l = k GT + tid (k < nmine) against the level-j table `tb` (already offset
+// by the slice base), two gates in flight.  Accumulators per bit value: X0/X1 collect W (x_b + c), Y0/Y1 collect
+// W (x_2 + c); G[0] = X0, G[1] = X1, G[2] = 2 Y1 - Y0.  s4 receives the canonical sums (flushed every 8 products).
+__device__ __forceinline__ void hot_gates(const bool IGN, const bool UPD, uint64_t *sW, const uint64_t *sC, const uint32_t *sI,
+                                          const uint64_t *tb, uint32_t j, uint32_t nmine, uint32_t tid, uint64_t r_prev,
+                                          uint64_t omr, uint64_t (&s4)[4]) {
+    constexpr uint32_t GT = F_WORKERS;
+    acc128 X0, X1, Y0, Y1; X0.clear(); X1.clear(); Y0.clear(); Y1.clear();
+    const uint32_t sh = j + 1;
+    auto one = [&](uint64_t &W, uint64_t cP, uint32_t idx, const ulonglong2 pr) {
+        if (UPD) W = fp61::mul(W, ((idx >> (j - 1)) & 1u) ? r_prev : omr);
+        uint64_t lo = pr.x, hi = pr.y;
+        if (IGN && (idx >> 31)) { lo = 0; hi = 0; }
+        const uint32_t bit = (idx >> j) & 1u;
+        const uint64_t mb = (bit ? hi : lo) + cP;                // < 2^61 + 2^62
+        const uint64_t m2 = 2 * hi + cP - lo;                    // 2 hi - lo + c + p  in (0, 2^63)
+        const uint64_t pl = W * mb, ph = fp61::mulhi(W, mb), ql = W * m2, qh = fp61::mulhi(W, m2);
+        if (bit) { mac1(X1, pl, ph); mac1(Y1, ql, qh); } else { mac1(X0, pl, ph); mac1(Y0, ql, qh); }
+    };
+    auto flush = [&]() {
+        s4[0] = fp61::add(s4[0], X0.value()); s4[1] = fp61::add(s4[1], X1.value());
+        s4[2] = fp61::add(s4[2], Y0.value()); s4[3] = fp61::add(s4[3], Y1.value());
+        X0.clear(); X1.clear(); Y0.clear(); Y1.clear();
+    };
+    uint32_t k = 0;
+    for (; k + 2 <= nmine; k += 2) {
+        const uint32_t l0 = k * GT + tid, l1 = l0 + GT;
+        uint64_t Wa = sW[l0], Wb = sW[l1];
+        const uint64_t ca = sC[l0], cb = sC[l1];
+        const uint32_t ia = sI[l0], ib = sI[l1];
+        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((ia & F_IDX_MASK) >> sh));
+        const ulonglong2 pb = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((ib & F_IDX_MASK) >> sh));
+        one(Wa, ca, ia, pa);
+        one(Wb, cb, ib, pb);
+        if (UPD) { sW[l0] = Wa; sW[l1] = Wb; }
+        if ((k & 6) == 6) flush();                               // 8 products per accumulator at most
+    }
+    if (k < nmine) {
+        const uint32_t l0 = k * GT + tid;
+        uint64_t Wa = sW[l0];
+        const uint32_t ia = sI[l0];
+        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((ia & F_IDX_MASK) >> sh));
+        one(Wa, sC[l0], ia, pa);
+        if (UPD) sW[l0] = Wa;
+    }
+    flush();
+}
+
 __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas, uint8_t *dyn,
                                            uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x, b = blockIdx.x;
@@ -224,34 +276,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 acc128 X, X1, Y, Y1; X.clear(); X1.clear(); Y.clear(); Y1.clear();
                 uint64_t s4[4] = {0, 0, 0, 0};                 // canonical running sums of X, X1, Y, Y1 (flushed every 8 products)
                 if (res && mode == F_MODE_SLICE) {
-                    // hot loop: state and table in shared memory (level 0: L2), two gates in flight per thread
-                    const uint64_t *tb = tab - base;
-                    const uint32_t sh = j + 1;
-                    uint32_t k = 0;
-                    for (; k + 2 <= nmine; k += 2) {
-                        const uint32_t l0 = k * GT + tid, l1 = l0 + GT;
-                        GateIn A, B;
-                        A.W = sW[l0]; A.cP = sC[l0]; A.idx = sI[l0];
-                        B.W = sW[l1]; B.cP = sC[l1]; B.idx = sI[l1];
-                        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((A.idx & F_IDX_MASK) >> sh));
-                        const ulonglong2 pb = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((B.idx & F_IDX_MASK) >> sh));
-                        gate_apply(A, pa, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
-                        gate_apply(B, pb, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
-                        if (upd) { sW[l0] = A.W; sW[l1] = B.W; }
-                        if ((k & 6) == 6) {      // 8 products per accumulator at most
-                            s4[0] = fp61::add(s4[0], X.value()); s4[1] = fp61::add(s4[1], X1.value());
-                            s4[2] = fp61::add(s4[2], Y.value()); s4[3] = fp61::add(s4[3], Y1.value());
-                            X.clear(); X1.clear(); Y.clear(); Y1.clear();
-                        }
-                    }
-                    if (k < nmine) {
-                        const uint32_t l0 = k * GT + tid;
-                        GateIn A;
-                        A.W = sW[l0]; A.cP = sC[l0]; A.idx = sI[l0];
-                        const ulonglong2 pa = *reinterpret_cast<const ulonglong2 *>(tb + 2 * (size_t)((A.idx & F_IDX_MASK) >> sh));
-                        gate_apply(A, pa, j, upd, r_prev, omr, has_ign, X, X1, Y, Y1);
-                        if (upd) sW[l0] = A.W;
-                    }
+                    // hot loop: state in shared memory; the table is level 0 in L2 (round 0) or a shared-memory buffer
+                    hot_gates(has_ign, upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                 } else {
                     for (uint32_t k = 0; k < nmine; k++) {
                         const uint32_t l = k * GT + tid, g = g0 + l;
@@ -278,12 +304,15 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                             X.clear(); X1.clear(); Y.clear(); Y1.clear();
                         }
                     }
+                    // totals -> per-bit sums: X0 = X - X1, Y0 = Y - Y1
+                    s4[1] = fp61::add(s4[1], X1.value()); s4[3] = fp61::add(s4[3], Y1.value());
+                    s4[0] = fp61::sub(fp61::add(s4[0], X.value()), s4[1]); s4[2] = fp61::sub(fp61::add(s4[2], Y.value()), s4[3]);
                 }
                 VC_TR(21);
                 if (!first) asm volatile("bar.sync 3, %0;" ::"r"((uint32_t)FT) : "memory");   // the reducer is done with round j-1's words
-                if (tid < ng) {                  // commit this worker's four sums (any representative < 2^62 will do)
+                if (tid < ng) {                  // commit this worker's four canonical sums X0, X1, Y0, Y1
                     ulonglong2 o0, o1;
-                    o0.x = s4[0] + X.value(); o0.y = s4[1] + X1.value(); o1.x = s4[2] + Y.value(); o1.y = s4[3] + Y1.value();
+                    o0.x = s4[0]; o0.y = s4[1]; o1.x = s4[2]; o1.y = s4[3];
                     cbuf[2 * tid] = o0; cbuf[2 * tid + 1] = o1;
                 }
             }
@@ -300,8 +329,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 }
                 if (!(ph == 1 && j + 1 == s)) asm volatile("bar.arrive 3, %0;" ::"r"((uint32_t)FT) : "memory");   // words consumed
                 const uint64_t x = fp61::fold128(Sh, Sl), x1 = fp61::fold128(S1h, S1l), y = fp61::fold128(Th, Tl), y1 = fp61::fold128(T1h, T1l);
-                const uint64_t t0 = warp_sum61(fp61::sub(x, x1)), t1 = warp_sum61(x1);
-                const uint64_t t2 = warp_sum61(fp61::sub(fp61::add(fp61::dbl(y1), y1), y));
+                const uint64_t t0 = warp_sum61(x), t1 = warp_sum61(x1);
+                const uint64_t t2 = warp_sum61(fp61::sub(fp61::dbl(y1), y));        // x, y here are the bit-0 sums
                 reducer_post(a, ep, t0, t1, t2, tr, pd);
             } else {
                 if (warp == 0) round_rendezvous(a, ep, fence, rslot, seed, ctr);   // ---- a6: rendezvous, then the challenge
