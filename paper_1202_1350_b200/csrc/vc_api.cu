@@ -157,6 +157,11 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const uint32_t d = c->d;
     const uint64_t n_in = 1ull << c->log_input;
+    if (c->schedule != 1) {                      // one cooperative launch for the whole evaluation when the circuit allows it
+        const int rc = vc::enqueue_eval_fused(c, d_input, d_outputs, st);
+        if (rc == VC_OK) { c->next_layer = 0; return VC_OK; }
+        if (rc != VC_ERR_STATE) return rc;
+    }
     VC_LAUNCH(VC_K_EVAL, vc::k_copy_input, grid_for(n_in, c->sm_count), vc::RED_BLOCK, 0, st, d_input, c->d_V[d], n_in, c->d_state);
     for (int i = (int)d - 1; i >= 0; i--) {
         const uint32_t n = 1u << c->logs[i];

@@ -65,6 +65,56 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     }
 }
 
+// ---- a1 in one launch: V_d <- input (checked canonical), then V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]) for
+// i = d-1..0 (all gates of a layer in parallel, layer after layer).  Grid-wide layers are separated by a
+// counter rendezvous; once the remaining layers are narrow CTA 0 finishes them alone behind block barriers.
+constexpr int EVAL_T = 1024;
+constexpr uint32_t EVAL_NARROW_LOG = 11;
+__device__ __forceinline__ void eval_grid_barrier(unsigned long long *cnt, uint32_t &gen) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        gen++;
+        __threadfence();
+        red_add(cnt, 1ull);
+        const unsigned long long want = (unsigned long long)gen * gridDim.x;
+        while (ld_acquire(cnt) < want) { }
+    }
+    __syncthreads();
+}
+__global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint32_t d, const uint64_t *in, uint64_t *out0,
+                                                          DevState *st, unsigned long long *cnt) {
+    const uint32_t tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
+    uint32_t gen = 0;
+    {
+        uint64_t *Vd = const_cast<uint64_t *>(L[d].V);
+        const uint64_t n = 1ull << L[d].log_n;
+        unsigned bad = 0;
+        for (uint64_t i = b * (uint64_t)EVAL_T + tid; i < n; i += (uint64_t)G * EVAL_T) {
+            const uint64_t w = in[i];
+            bad |= (w >= fp61::P);
+            Vd[i] = w;
+        }
+        if (bad) atomicOr(&st->flags, 1u);
+    }
+    bool solo = false;                            // CTA 0 alone from the first layer whose inputs and outputs are narrow
+    for (int i = (int)d - 1; i >= 0; i--) {
+        const uint32_t n = 1u << L[i].log_n;
+        const bool narrow = L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1;
+        if (!solo) eval_grid_barrier(cnt, gen); else __syncthreads();
+        if (narrow && !solo) { solo = true; if (b != 0) return; }
+        const uint8_t *__restrict__ type = L[i].type;
+        const uint32_t *__restrict__ in1 = L[i].in1, *__restrict__ in2 = L[i].in2;
+        const uint64_t *Vb = L[i + 1].V;
+        uint64_t *Vo = const_cast<uint64_t *>(L[i].V);
+        const uint32_t start = solo ? tid : b * EVAL_T + tid, stride = solo ? EVAL_T : G * EVAL_T;
+        for (uint32_t g = start; g < n; g += stride) {
+            const uint64_t v = gate_f(type[g], __ldcg(Vb + in1[g]), __ldcg(Vb + in2[g]));
+            Vo[g] = v;
+            if (i == 0 && out0) out0[g] = v;
+        }
+    }
+}
+
 constexpr size_t F_SMEM_MAX = 227 * 1024;
 
 struct FusedHost {
@@ -72,6 +122,8 @@ struct FusedHost {
     CtaPlan *d_cta = nullptr;
     unsigned long long *d_slots = nullptr;
     uint64_t *d_stamps = nullptr, *d_C = nullptr, *d_Tg = nullptr;
+    unsigned long long *d_evcnt = nullptr;
+    bool eval_ok = false;
     int grid = 0;
     size_t smem = 0;
 };
@@ -214,6 +266,19 @@ int fused_init(vc_circuit *c) {
     if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_C, max_gates * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_Tg, (size_t)(2u << F_TLOG) * 8) != cudaSuccess) return VC_ERR_NOMEM;
+    if (cudaMalloc(&fh.d_evcnt, 64) != cudaSuccess) return VC_ERR_NOMEM;
+    {   // the one-launch evaluation needs: a co-resident grid, and narrow layers only at the output end
+        int eper = 0;
+        bool ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eper, k_eval_all, EVAL_T, 0) == cudaSuccess && eper >= 1;
+        bool seen_narrow = false;
+        for (int i = (int)c->d - 1; i >= 0 && ok; i--) {
+            const bool narrow = c->logs[i] <= EVAL_NARROW_LOG && c->logs[i + 1] <= EVAL_NARROW_LOG + 1;
+            if (seen_narrow && !narrow) ok = false;
+            seen_narrow = seen_narrow || narrow;
+        }
+        (void)cudaGetLastError();
+        fh.eval_ok = ok;
+    }
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
@@ -228,7 +293,7 @@ void fused_free(const vc_circuit *c) {
     for (size_t i = 0; i < g_fused.size(); i++)
         if (g_fused[i].first == c) {
             FusedHost &f = g_fused[i].second;
-            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg);
+            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg); cudaFree(f.d_evcnt);
             g_fused.erase(g_fused.begin() + i);
             return;
         }
@@ -258,6 +323,22 @@ int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st) {
     if (!fh) return VC_ERR_STATE;
     if (cudaStreamSynchronize(st) != cudaSuccess) return VC_ERR_CUDA;
     return cudaMemcpy(h, fh->d_stamps, (size_t)(c->d + 1) * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? VC_OK : VC_ERR_CUDA;
+}
+
+// a1 in one cooperative launch; returns VC_ERR_STATE when this circuit must use the per-layer kernels instead
+int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, cudaStream_t st) {
+    FusedHost *fh = find(c);
+    if (!fh || !fh->eval_ok) return VC_ERR_STATE;
+    if (cudaMemsetAsync(fh->d_evcnt, 0, 8, st) != cudaSuccess) return VC_ERR_CUDA;
+    const LayerPlan *L = fh->d_plan; uint32_t d = c->d; DevState *S = c->d_state; unsigned long long *cnt = fh->d_evcnt;
+    void *params[] = {&L, &d, &d_input, &d_outputs, &S, &cnt};
+    cudaEvent_t ea = nullptr, eb = nullptr;
+    if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_eval_all, dim3(fh->grid), dim3(EVAL_T), params, 0, st);
+    if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_EVAL, ea, eb); }
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    return VC_OK;
 }
 
 int fused_trace(const vc_circuit *c, uint64_t *h, uint32_t n_words, cudaStream_t st) {
