@@ -22,7 +22,7 @@ namespace vc {
 constexpr int FT = 512;                  // threads per CTA (128 registers each)
 constexpr int F_TLOG = 10;               // the fully shared part of a fold table has 2^min(s, F_TLOG) entries
 constexpr int F_EQLOG = 10;              // eq tables are built in halves of at most 2^10 entries
-constexpr int F_SMALL_N_LOG = 9;         // single-CTA path: gates <= 2^9 (one per thread) ...
+constexpr int F_SMALL_N_LOG = 8;         // single-CTA path: gates <= 2^8 (one per worker thread) ...
 constexpr int F_SMALL_T_LOG = 12;        // ... and table <= 2^12 words
 constexpr int F_SLOT_WORDS = 128;        // one rendezvous slot: up to 64 values x (lo,hi)
 constexpr int F_RING = 8;                // slots are recycled two epochs ahead and converted up to two epochs late

@@ -45,93 +45,107 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
                                             uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t si = a.L[layer].log_n, s = a.L[layer + 1].log_n;
-    const uint32_t n = 1u << si, nb = 1u << s;
-    uint32_t nthr = 32;
-    { const uint32_t need = n > (nb >> 1) ? n : (nb >> 1); while (nthr < need && nthr < (uint32_t)FT) nthr <<= 1; }
+    const uint32_t n = 1u << si, nb = 1u << s;                   // n <= 2^F_SMALL_N_LOG <= 256, nb <= 2^F_SMALL_T_LOG
+    uint64_t *Vs = reinterpret_cast<uint64_t *>(dyn);            // level 0: V_{i+1}
+    uint64_t *X = Vs + (1u << F_SMALL_T_LOG);                     // odd levels
+    uint64_t *Y = X + (1u << (F_SMALL_T_LOG - 1));                // even levels >= 2
+    ulonglong2 *cbuf = reinterpret_cast<ulonglong2 *>(Y + (1u << (F_SMALL_T_LOG - 2)));   // [2][256] committed products
+    uint64_t *sred = reinterpret_cast<uint64_t *>(cbuf + 2 * 256);
+    uint64_t *scratch = sred + 32;
     __syncthreads();                                             // bookkeeping of the previous layer is settled
-    if (tid < nthr) {
-        uint64_t *Vs = reinterpret_cast<uint64_t *>(dyn);        // level 0: V_{i+1}
-        uint64_t *X = Vs + (1u << F_SMALL_T_LOG);                 // odd levels
-        uint64_t *Y = X + (1u << (F_SMALL_T_LOG - 1));            // even levels >= 2
-        uint64_t *sred = Y + (1u << (F_SMALL_T_LOG - 2));         // [parity][warp][4]
-        uint64_t *scratch = sred + 2 * 32 * 4;
-        const uint32_t nw = nthr >> 5;
-        const uint64_t *Vg = a.L[layer + 1].V;
-        for (uint32_t u = tid; u < nb; u += nthr) Vs[u] = Vg[u];
-        const bool live = tid < n;
-        uint64_t P = live ? eq_direct(tid, cx.z, 0, si) : 0;     // a3: beta(z, g) by direct product
-        uint32_t i1 = 0, i2 = 0, t = VC_RELAY;
-        if (live) { i1 = a.L[layer].in1[tid]; i2 = a.L[layer].in2[tid]; t = a.L[layer].type[tid]; }
-        uint32_t ctr = (uint32_t)cx.ctr;
-        const uint64_t seed = cx.seed;
-        bar_n(nthr);
-        if (layer == 0) {                                        // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
-            const uint64_t v = warp_sum61(live ? fp61::mul(P, a.L[0].V[tid]) : 0);
-            if (lane == 0) sred[warp * 4] = v;
-            bar_n(nthr);
-            if (warp == 0) {
-                const uint64_t tot = warp_sum61(lane < nw ? sred[lane * 4] : 0);
-                if (lane == 0) cx.claim = tot;
-            }
-            bar_n(nthr);
+    const uint64_t *Vg = a.L[layer + 1].V;
+    for (uint32_t u = tid; u < nb; u += FT) Vs[u] = __ldcg(Vg + u);
+    const bool live = tid < n;
+    uint64_t P = live ? eq_direct(tid, cx.z, 0, si) : 0;         // a3: beta(z, g) by direct product
+    uint32_t i1 = 0, i2 = 0, t = VC_RELAY;
+    if (live) { i1 = a.L[layer].in1[tid]; i2 = a.L[layer].in2[tid]; t = a.L[layer].type[tid]; }
+    uint32_t ctr = (uint32_t)cx.ctr;
+    const uint64_t seed = cx.seed;
+    __syncthreads();
+    if (layer == 0) {                                            // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
+        const uint64_t v = warp_sum61(live ? fp61::mul(P, a.L[0].V[tid]) : 0);
+        if (lane == 0) sred[warp] = v;
+        __syncthreads();
+        if (warp == 0) {
+            const uint64_t tot = warp_sum61(lane < (uint32_t)FT / 32 ? sred[lane] : 0);
+            if (lane == 0) cx.claim = tot;
         }
-        uint32_t par = 0;
-        VC_TR(1);
-        for (int phase = 1; phase <= 2; phase++) {
-            const uint32_t idx = phase == 1 ? i1 : i2;
-            uint64_t W, c; uint32_t ign;
-            gate_state(phase, t, P, phase == 1 ? Vs[i2] : cx.v1, W, c, ign);
-            if (!live) { W = 0; c = 0; }
-            for (uint32_t j = 0; j < s; j++) {
-                const uint64_t *tab = j == 0 ? Vs : ((j & 1) ? X : Y);
-                const uint32_t bit = (idx >> j) & 1u, u = idx >> (j + 1);
+        __syncthreads();
+    }
+    uint32_t par = 0;
+    VC_TR(1);
+    for (int phase = 1; phase <= 2; phase++) {
+        const uint32_t idx = phase == 1 ? i1 : i2;
+        uint64_t W = 0, c = 0; uint32_t ign = 0;
+        if (live) gate_state(phase, t, P, phase == 1 ? Vs[i2] : cx.v1, W, c, ign);
+        const uint64_t cP = c + fp61::P;
+        for (uint32_t j = 0; j < s; j++) {
+            const uint64_t *tab = j == 0 ? Vs : ((j & 1) ? X : Y);
+            const uint32_t bit = (idx >> j) & 1u;
+            if (live) {                                          // a4: this thread's gate; its two products are committed
+                const uint32_t u = idx >> (j + 1);
                 uint64_t lo = tab[2 * u], hi = tab[2 * u + 1];
                 if (ign) { lo = 0; hi = 0; }
-                acc128 A, A1, B, B1; A.clear(); A1.clear(); B.clear(); B1.clear();
-                gate_mac(W, c, bit, lo, hi, A, A1, B, B1);
-                uint64_t g[3];
-                gate_fin(A, A1, B, B1, g);
-                uint64_t *pr = sred + par * 128;
-#pragma unroll
-                for (int k = 0; k < 3; k++) { g[k] = warp_sum61(g[k]); if (lane == 0) pr[warp * 4 + k] = g[k]; }
-                VC_TR(2);
-                bar_n(nthr);                                     // the message of this round is complete
-                VC_TR(3);
-                if (warp == 0) {                                 // transcript, off the critical path of the other warps
-#pragma unroll
-                    for (int k = 0; k < 3; k++) {
-                        const uint64_t tot = warp_sum61(lane < nw ? pr[lane * 4 + k] : 0);
-                        if (lane == 0) tr[k] = tot;
-                    }
+                const uint64_t mb = (bit ? hi : lo) + cP, m2 = 2 * hi + cP - lo;
+                ulonglong2 o;
+                o.x = fp61::fold128(fp61::mulhi(W, mb), W * mb) | ((uint64_t)bit << 63);
+                o.y = fp61::fold128(fp61::mulhi(W, m2), W * m2);
+                cbuf[par * 256 + tid] = o;
+            }
+            VC_TR(2);
+            __syncthreads();                                     // every contribution to message j is committed
+            VC_TR(3);
+            if (warp == 15) {                                    // a5 off the critical path: G[0..2] -> transcript
+                const ulonglong2 *cb = cbuf + par * 256;
+                uint64_t X0l = 0, X1l = 0, Y0l = 0, Y1l = 0; uint32_t X0h = 0, X1h = 0, Y0h = 0, Y1h = 0;
+                for (uint32_t i = lane; i < n; i += 32) {
+                    const ulonglong2 q = cb[i];
+                    const uint32_t b1 = (uint32_t)(q.x >> 63);
+                    const uint64_t v1 = q.x & ~(1ull << 63);
+                    add_c(X0l, X0h, v1, b1 ^ 1u); add_c(X1l, X1h, v1, b1);
+                    add_c(Y0l, Y0h, q.y, b1 ^ 1u); add_c(Y1l, Y1h, q.y, b1);
                 }
-                tr += 3; par ^= 1;
-                const uint64_t r = fp61::draw(seed, ctr); ctr++;   // a6: challenge, weight update, fold
-                const uint64_t f = bit ? r : fp61::sub(1, r);
-                W = fp61::mul(W, f); P = fp61::mul(P, f);
-                uint64_t *out = ((j + 1) & 1) ? X : Y;
+                const uint64_t t0 = warp_sum61(fp61::fold128(X0h, X0l)), t1 = warp_sum61(fp61::fold128(X1h, X1l));
+                const uint64_t y0 = fp61::fold128(Y0h, Y0l), y1 = fp61::fold128(Y1h, Y1l);
+                const uint64_t t2 = warp_sum61(fp61::sub(fp61::dbl(y1), y0));
+                if (lane < 3) tr[lane] = lane == 0 ? t0 : (lane == 1 ? t1 : t2);
+            } else {                                             // a6: challenge, weight update, fold
                 const uint32_t half = nb >> (j + 1);
-                for (uint32_t v = tid; v < half; v += nthr) out[v] = fold2(tab[2 * v], tab[2 * v + 1], r);
-                if (tid == 0) { if (phase == 1) cx.r1[j] = r; else cx.r2[j] = r; }
+                if (tid < n || tid < half) {                     // idle warps go straight to the barrier
+                    const uint64_t r = fp61::draw(seed, ctr);
+                    if (live) {
+                        const uint64_t f = bit ? r : fp61::sub(1, r);
+                        W = fp61::mul(W, f); P = fp61::mul(P, f);
+                    }
+                    uint64_t *out = ((j + 1) & 1) ? X : Y;
+                    for (uint32_t v = tid; v < half; v += F_WORKERS) out[v] = fold2(tab[2 * v], tab[2 * v + 1], r);
+                    if (tid == 0) { if (phase == 1) cx.r1[j] = r; else cx.r2[j] = r; }
+                }
                 VC_TR(4);
-                bar_n(nthr);
+                bar_workers();
                 VC_TR(5);
             }
-            const uint64_t vend = ((s & 1) ? X : Y)[0];           // level s: V~_{i+1}(r1) resp. (r2)
-            if (tid == 0) { if (phase == 1) cx.v1 = vend; else cx.v2 = vend; }
-            // P now equals beta(z,g) eq(in1[g], r1): the plain weight phase 2 starts from
-            bar_n(nthr);
+            ctr++; tr += 3; par ^= 1;
         }
-        if (tid == 0) cx.ctr = ctr;
-        VC_TR(6);
-        if (s > 1) line_partials(Vs, s, cx, pas, scratch, 0, 1, tid, nthr, fused_line_tb(s, nthr));   // a7 (its first barrier publishes cx.ctr)
-        else bar_n(nthr);
-        VC_TR(7);
-        line_finish(s, cx, invfact, tr, true, tid);
-        VC_TR(8);
+        __syncthreads();                                         // the reducer is done; level s and r[] are visible to all
+        const uint64_t vend = ((s & 1) ? X : Y)[0];               // level s: V~_{i+1}(r1) resp. (r2)
+        if (tid == 0) { if (phase == 1) cx.v1 = vend; else cx.v2 = vend; }
+        // P now equals beta(z,g) eq(in1[g], r1): the plain weight phase 2 starts from
+        __syncthreads();
     }
+    if (tid == 0) cx.ctr = ctr;
+    VC_TR(6);
+    uint32_t nthr = 32;
+    while (nthr < (nb >> 3) && nthr < (uint32_t)FT) nthr <<= 1;   // the line restriction wants 2^(s-3) threads
+    __syncthreads();
+    if (tid < nthr && s > 1) line_partials(Vs, s, cx, pas, scratch, 0, 1, tid, nthr, fused_line_tb(s, nthr));   // a7
+    __syncthreads();
+    VC_TR(7);
+    line_finish(s, cx, invfact, tr, true, tid);
+    VC_TR(8);
     __syncthreads();
 }
 
-constexpr size_t F_SMALL_BYTES = (F_SMALL_WORDS + 13 * 12 + 2 + 512 * 13 + 256 * 13 + 2 + 64) * 8;   // + line scratch, s <= 12
+constexpr size_t F_SMALL_BYTES = (F_SMALL_WORDS + 2 * 256 * 2 + 32 + 13 * 12 + 2 + 512 * 13 + 256 * 13 + 2 + 64) * 8;   // + commit + line scratch, s <= 12
 
 }  // namespace vc
