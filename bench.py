@@ -176,8 +176,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     k = args.config
     c = W.config(k)
-    if rank > 0:                                   # replicas: same circuit, another seeded input of the same recipe
-        c.input = np.random.default_rng(W.data_seed(k) + rank).permutation(c.input)
+    from paper_1202_1350_b200 import replicas
+    c.input = replicas.replica_input(c.input, W.data_seed(k), rank)   # replicas: same circuit, another seeded input
     seed = W.challenge_seed(k)
     L = vc.lib()
     gc = vc.Circuit(c)
@@ -233,13 +233,10 @@ def run_ours(args):
         e2e_ms += a.elapsed_time(b)
     barrier()
     clocks = sampler.summary()
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(t[0]), float(t[1])
+    total_ms, e2e_ms = replicas.max_over_ranks([total_ms, e2e_ms], device="cuda")
     ms_per_step = total_ms / args.steps
-    value = c.gates * world / (ms_per_step * 1e-3)
-    e2e_value = c.gates * world / (e2e_ms / args.steps * 1e-3)
+    value = replicas.whole_job_value(c.gates, world, ms_per_step)
+    e2e_value = replicas.whole_job_value(c.gates, world, e2e_ms / args.steps)
 
     if rank == 0:
         # ---- per-kernel-kind timing (CUDA events inside the library, on the launching stream), one extra step

@@ -27,6 +27,15 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     }
     if (tid <= MAX_VARS) invfact[tid] = a.st->invfact[tid];
     build_pascal(pas, tid);
+#ifdef VC_POISON                                   // debug build: uninitialised shared-memory reads become loud
+    {
+        uint32_t dsz;
+        asm volatile("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dsz));
+        for (uint32_t i = tid; i < (dsz - (uint32_t)F_FIXED_BYTES) / 8; i += FT) reinterpret_cast<uint64_t *>(dyn)[i] = 0xDEADBEEFDEADBEEFull;
+        if (tid < 128) cx.red[tid] = 0xDEADBEEFDEADBEEFull;
+        if (tid < MAX_VARS) cx.acc[tid] = 0xDEADBEEFDEADBEEFull;
+    }
+#endif
     if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; cx.pad = 0; cx.pend_tr = nullptr; cx.pend_slot = 0; }
     __syncthreads();
     uint64_t *tr = a.tr;

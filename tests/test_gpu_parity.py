@@ -93,6 +93,8 @@ RANDOM_CASES = [
     ([0, 1, 2, 3, 4, 5], 6, 9), ([4, 6, 5], 7, 10), ([6, 3], 5, 12),
     ([9, 12, 10, 13], 11, 13),          # several tiles of every kernel + ragged sizes between layers
     ([14, 11, 15], 13, 14),
+    ([12, 17, 8], 9, 15),               # 2^12 gates wired at random into a 2^17 table: tables materialised in L2 (F_MODE_GLOBAL)
+    ([21, 17], 10, 16),                 # 2^21 gates: state in global scratch (non-resident) + F_MODE_GLOBAL
 ]
 
 
