@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (tid < MAX_VARS) cx.acc[tid] = 0xDEADBEEFDEADBEEFull;
     }
 #endif
-    if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; cx.pad = 0; cx.pend_tr = nullptr; cx.pend_slot = 0; }
+    if (tid == 0) { cx.epoch = a.st->bar_gen; cx.v1 = 0; cx.v2 = 0; cx.pad = 0; }
     __syncthreads();
     uint64_t *tr = a.tr;
     bool handoff = false;                         // CTA 0 ran narrow layers alone: publish its state first
@@ -152,7 +152,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
     lp.kind = (si <= (uint32_t)F_SMALL_N_LOG && s <= (uint32_t)F_SMALL_T_LOG) ? 0 : 1;
     lp.has_relay = 0;
     for (uint8_t t : c->h_type[i]) if (t == VC_RELAY) { lp.has_relay = 1; break; }
-    lp.thin = 0; lp.resident = 0; lp.cap = 0; lp.gthr = FT; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
+    lp.thin = 0; lp.resident = 0; lp.cap = 0; lp.mode[0] = lp.mode[1] = F_MODE_GLOBAL; lp.K[0] = lp.K[1] = 0;
     lp.xw = lp.yw = 0; lp.off_tab = lp.off_scr = lp.off_commit = 0;
     if (lp.kind == 0) { smem_need = std::max(smem_need, F_FIXED_BYTES + F_SMALL_BYTES); return; }
     // gates in units of 32, spread evenly over the CTAs
@@ -174,7 +174,6 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         }
     }
     const size_t cap = (size_t)((ngmax + FT - 1) / FT) * FT;
-    lp.gthr = FT;                                // one gate per thread first: thin layers are bound by the per-gate latency chain
     const size_t state = cap * 20;
     // fold buffers: odd levels in X, even levels in Y; slices exist for levels 1..K-1
     auto buf_words = [&](int ph, size_t &xw, size_t &yw) {

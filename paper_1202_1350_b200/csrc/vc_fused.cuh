@@ -10,10 +10,12 @@
 //     costs 3 wide multiplies per gate-round;
 //   * fold tables live in shared memory: each CTA folds the slice its gates read (levels < K) and, from level K on,
 //     the whole (<= 2^10-entry) table, redundantly; level K-1 is published through L2 once per phase;
-//   * the three round values are all-reduced through one L2 line per round (red.add + polling), after which every
-//     CTA draws the challenge itself: one grid rendezvous per round, no kernel launch, no host round-trip.
-// Challenges are only ever used AFTER the message they answer has been completely reduced (causality of the
-// interactive protocol), although the seeded generator would allow drawing them earlier.
+//   * a round ends in one grid rendezvous on a count word in L2 (atom.add + polling by one lane per CTA); warp 15 of
+//     every CTA (the "reducer") sums the CTA's committed contributions mod p and adds them to the round's six data
+//     words with red.add while the next round is already running; no kernel launch, no host round-trip.
+// A challenge is only ever used AFTER every contribution to the message it answers has been committed (causality of
+// the interactive protocol), although the seeded generator would allow drawing it earlier; what is
+// pipelined is the summation of the committed contributions into the three transcript words.
 #pragma once
 #include "vc_kernels.cuh"
 
@@ -47,7 +49,6 @@ struct LayerPlan {
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
     uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
     uint32_t cap;                        // state capacity in gates (multiple of FT)
-    uint32_t gthr;                       // threads per CTA that own gates (multiple of 32, <= FT)
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
     uint32_t xw, yw;                     // words of the two fold buffers
@@ -74,8 +75,6 @@ struct FusedCtx {            // block-shared bookkeeping, replicated in every CT
     uint64_t G[4];
     uint64_t seed, ctr, claim, v1, v2;
     uint32_t epoch, pad;
-    uint64_t *pend_tr;       // CTA 0: transcript position of the round whose slot is not converted yet (or null)
-    uint32_t pend_slot, pad2;
 };
 
 // fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS, then Pascal's triangle C(n,k),
@@ -221,12 +220,6 @@ __device__ __noinline__ void grid_allreduce(FusedCtx &cx, const FusedArgs &a, ui
     __syncthreads();
 }
 
-// ---- the per-round fast path: per-warp partials (3 words each) sit in cx.red[w*4 + k], w < nw.  Warp 0 combines
-// them and posts the CTA totals as six (value | count) words; lane 0 alone waits until word 0 carries every CTA's
-// count: that is the rendezvous ("message complete").  Nobody needs the grid totals to go on, so they are not read
-// back here: warp 2 of CTA 0 turns the slot of the PREVIOUS round into transcript words while the next round runs
-// (transcript_flush does it for the last round of a phase).  The challenge that answers the message, r = H(seed,
-// ctr), is generated by warp 0 while it waits and handed out through *rslot only after the rendezvous.
 __device__ __forceinline__ unsigned long long atom_add(unsigned long long *p, unsigned long long v) {
     unsigned long long r;
     asm volatile("atom.relaxed.gpu.global.add.u64 %0, [%1], %2;" : "=l"(r) : "l"(p), "l"(v) : "memory");
@@ -236,64 +229,6 @@ __device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long lon
     unsigned long long v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
-}
-// converts a completed slot (6 words) into G[0..2] -> tr[0..2]; called by one full warp of CTA 0
-__device__ __forceinline__ void slot_to_transcript(const unsigned long long *slot, uint64_t *tr, uint32_t lane) {
-    uint64_t got = 0;
-    if (lane < 6) {
-        const uint64_t want = (uint64_t)gridDim.x;
-        unsigned long long w;
-        while (((w = ld_relaxed(slot + lane)) >> 48) != want) { }
-        got = w & F_VAL_MASK;
-    }
-    const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
-    if (lane < 6 && !(lane & 1)) tr[lane >> 1] = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
-}
-__device__ __forceinline__ void transcript_flush(FusedCtx &cx, const FusedArgs &a) {   // CTA 0, warp 2 only
-    if (cx.pend_tr) {
-        slot_to_transcript(a.slots + (size_t)cx.pend_slot * F_SLOT_WORDS, cx.pend_tr, threadIdx.x & 31);
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0) cx.pend_tr = nullptr;
-    }
-}
-__device__ __forceinline__ void round_allreduce(FusedCtx &cx, const FusedArgs &a, uint32_t nw, bool fence, uint64_t *tr,
-                                                uint64_t *rslot, uint64_t seed, uint32_t ctr) {
-    const uint32_t tid = threadIdx.x, lane = tid & 31;
-    const uint32_t ep = cx.epoch;        // last written before the trailing barrier of the previous rendezvous
-    __syncthreads();
-    VC_TR(31);
-    if (tid < 32) {
-        unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
-        const uint64_t t0 = warp_sum61(lane < nw ? cx.red[lane * 4 + 0] : 0);
-        const uint64_t t1 = warp_sum61(lane < nw ? cx.red[lane * 4 + 1] : 0);
-        const uint64_t t2 = warp_sum61(lane < nw ? cx.red[lane * 4 + 2] : 0);
-        const uint64_t r = fp61::draw(seed, ctr);
-        VC_TR(32);
-        if (lane < 6) {
-            const uint64_t v = lane < 2 ? t0 : (lane < 4 ? t1 : t2);
-            const uint64_t part = ((lane & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE;
-            if (fence) __threadfence();
-            if (lane == 0) {
-                const uint64_t want = (uint64_t)gridDim.x;
-                if ((atom_add(slot, part) >> 48) + 1 != want)
-                    while ((ld_relaxed(slot) >> 48) != want) { }
-                if (fence) __threadfence();
-            } else {
-                red_add(slot + lane, part);
-            }
-        }
-        VC_TR(33);
-        if (lane == 0) { cx.epoch = ep + 1; *rslot = r; }
-    } else if (blockIdx.x == 0) {
-        if (tid >= 64 && tid < 96) {     // transcript of the previous round, then remember this one
-            transcript_flush(cx, a);
-            if (lane == 0) { cx.pend_slot = ep % F_RING; cx.pend_tr = tr; }
-        } else if (tid >= 128 && tid < 128 + F_SLOT_WORDS) {
-            (a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS)[tid - 128] = 0ull;
-            __threadfence();
-        }
-    }
-    __syncthreads();
 }
 
 // ---- warp-specialised rounds (vc_fused_thin.cuh, vc_fused_wide.cuh): warps 0..14 work, warp 15 reduces.

@@ -23,24 +23,6 @@ __device__ __forceinline__ void gate_state(int phase, uint32_t t, uint64_t P, ui
     else { W = P; c = phase == 1 ? 0 : other; ign = phase == 1 ? 0u : 1u; }
 }
 
-// One gate's two products of a round, accumulated without reduction:
-//   X += W (x_b + c)      and, if b, X1 += the same           ->  G[0] = X - X1,  G[1] = X1
-//   Y += W (x_2 + c)      and, if b, Y1 += the same           ->  G[2] = 2 Y1 - (Y - Y1)      (chi(1,2) = 2, chi(0,2) = -1)
-// with x_b = b ? hi : lo and x_2 = 2 hi - lo.  Operands stay below 2^63, products below 2^124: 8 of them fit 128 bits.
-__device__ __forceinline__ void gate_mac(uint64_t W, uint64_t c, uint32_t b, uint64_t lo, uint64_t hi, acc128 &X, acc128 &X1,
-                                         acc128 &Y, acc128 &Y1) {
-    const uint64_t mb = (b ? hi : lo) + c;                       // < 2^62
-    const uint64_t m2 = 2 * hi + (fp61::P - lo) + c;             // < 2^63
-    fp61::mac2(X.lo, X.hi, X1.lo, X1.hi, W, mb, b);
-    fp61::mac2(Y.lo, Y.hi, Y1.lo, Y1.hi, W, m2, b);
-}
-__device__ __forceinline__ void gate_fin(const acc128 &X, const acc128 &X1, const acc128 &Y, const acc128 &Y1, uint64_t (&g)[3]) {
-    const uint64_t x = X.value(), x1 = X1.value(), y = Y.value(), y1 = Y1.value();
-    g[0] = fp61::sub(x, x1);
-    g[1] = x1;
-    g[2] = fp61::sub(fp61::add(fp61::dbl(y1), y1), y);
-}
-
 __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas, uint8_t *dyn,
                                             uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;

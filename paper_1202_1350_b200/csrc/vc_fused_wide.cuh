@@ -81,7 +81,8 @@ __device__ __forceinline__ void mac1(acc128 &A, uint64_t pl, uint64_t ph) {
 // The resident hot loop: this thread's gates l = k GT + tid (k < nmine) against the level-j table `tb` (already offset
 // by the slice base), two gates in flight.  Accumulators per bit value: X0/X1 collect W (x_b + c), Y0/Y1 collect
 // W (x_2 + c); G[0] = X0, G[1] = X1, G[2] = 2 Y1 - Y0.  s4 receives the canonical sums (flushed every 8 products).
-__device__ __forceinline__ void hot_gates(const bool IGN, const bool UPD, uint64_t *sW, const uint64_t *sC, const uint32_t *sI,
+template <bool IGN>
+__device__ __forceinline__ void hot_gates(const bool UPD, uint64_t *sW, const uint64_t *sC, const uint32_t *sI,
                                           const uint64_t *tb, uint32_t j, uint32_t nmine, uint32_t tid, uint64_t r_prev,
                                           uint64_t omr, uint64_t (&s4)[4]) {
     constexpr uint32_t GT = F_WORKERS;
@@ -277,7 +278,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 uint64_t s4[4] = {0, 0, 0, 0};                 // canonical running sums of X, X1, Y, Y1 (flushed every 8 products)
                 if (res && mode == F_MODE_SLICE) {
                     // hot loop: state in shared memory; the table is level 0 in L2 (round 0) or a shared-memory buffer
-                    hot_gates(has_ign, upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
+                    if (has_ign) hot_gates<true>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
+                    else hot_gates<false>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                 } else {
                     for (uint32_t k = 0; k < nmine; k++) {
                         const uint32_t l = k * GT + tid, g = g0 + l;
