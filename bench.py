@@ -273,8 +273,16 @@ def run_ours(args):
         t_hbm = counts["bytes"] / (peak * 1e9)
         t_alu = counts["modmul"] / best
         roof_ms = max(t_hbm, t_alu) * 1e3
+        traffic = None                           # dram bytes of the dominant kernel, from the committed ncu capture
+        try:
+            with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+                tj = json.load(f)
+            if k == 2 and args.schedule == 0 and dom == "fused_wide":
+                traffic = int(tj["dram_bytes_read"]) + int(tj["dram_bytes_write"])
+        except Exception:
+            pass
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": None, "peak_source": peak_src, "what": dom_desc,
+                    "traffic": traffic, "peak_source": peak_src, "what": dom_desc,
                     "kernel_share_of_step": prof[dom]["ms"] / prof_total, "per_kind": prof,
                     "step": {"algorithmic_bytes": counts["bytes"], "algorithmic_modmul": counts["modmul"],
                              "hbm_bound_ms": t_hbm * 1e3, "modmul_rate_per_s": best, "alu_bound_ms": t_alu * 1e3,
