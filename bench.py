@@ -288,6 +288,24 @@ def run_ours(args):
                              "hbm_bound_ms": t_hbm * 1e3, "modmul_rate_per_s": best, "alu_bound_ms": t_alu * 1e3,
                              "roofline_ms": roof_ms, "frac": roof_ms / ms_per_step,
                              "frac_at_8TBps": counts["bytes"] / 8e12 * 1e3 / ms_per_step}}
+        # ---- NEXT-1: the verifier with its O(S) sums on the GPU, beside the library's host verifier
+        # (outside the timed region; wall clock around the synchronous calls)
+        verifier = None
+        try:
+            vt = []
+            for _ in range(5):
+                t0 = time.perf_counter()
+                verdict = gc.verify_device(seed, stream=stream)
+                vt.append((time.perf_counter() - t0) * 1e3)
+            h_out, h_tr = gc.outputs().copy(), gc.transcript().copy()
+            t0 = time.perf_counter()
+            verdict_host = gc.verify(c.input, h_out, seed, h_tr)
+            host_ms = (time.perf_counter() - t0) * 1e3
+            verifier = {"device_ms": float(np.median(vt)), "host_ms": host_ms, "accept": bool(verdict[0]),
+                        "agree": verdict == verdict_host, "kernels": c.d + 2,
+                        "what": "vc_verify_transcript_device (d+2 kernels + host round checks) vs vc_verify_transcript (1 host thread)"}
+        except Exception as e:                       # never let the extra line break the bench contract
+            verifier = {"error": str(e)}
         # ---- the oracle, timed beside it on the host cores (bounded: one whole proof of config 2 is ~15 s)
         cpu = None
         if not args.no_cpu_baseline:
@@ -315,7 +333,7 @@ def run_ours(args):
                 "clocks": clocks, "gpu_launches": launches,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(c.input.nbytes),
                         "d2h_bytes_per_step": int(8 * (gc.n_out + gc.words)), "ms_per_step": e2e_ms / args.steps},
-                "roofline": roofline, "cpu_baseline": cpu}
+                "roofline": roofline, "cpu_baseline": cpu, "verifier": verifier}
         print(json.dumps(line), flush=True)
     gc.close()
     if world > 1:

@@ -85,6 +85,19 @@ int vc_verify_transcript(const vc_circuit *c, const uint64_t *h_input, const uin
                          const uint64_t *h_transcript, uint64_t n_words, int *accept, uint32_t *fail_layer,
                          uint32_t *fail_round);
 
+/* vc_verify_transcript_device — the same verifier with its O(S) sums on the GPU (
+ * PAPER.md:127 §4.1.2: one chi-weighted term per input element, reduced in F_p).  Three kinds of sums
+ * run as kernels, all enqueued at once on cuda_stream: the start claim V~_0(z_0) of the claimed outputs, the four
+ * per-type wiring sums of every layer, and the closing extension V~_d(z_d) of the input; the O(rounds) checks then run
+ * on the host over the transcript (copied back: 7s+1 words per layer).  Same acceptance rule, same
+ * (fail_layer, fail_round) and same error codes as vc_verify_transcript.
+ *   d_input, d_outputs, d_transcript: DEVICE pointers (read); accept, fail_layer, fail_round: HOST (written).
+ * Synchronises cuda_stream before returning.  Scratch for the sums is allocated on the first call for a circuit
+ * (VC_ERR_NOMEM if that fails) and released by vc_circuit_free. */
+int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *d_input, const uint64_t *d_outputs, uint64_t seed,
+                                const uint64_t *d_transcript, uint64_t n_words, int *accept, uint32_t *fail_layer,
+                                uint32_t *fail_round, void *cuda_stream);
+
 void vc_circuit_free(vc_circuit *c);
 const char *vc_strerror(int code);
 uint64_t vc_transcript_words(const vc_circuit *c, uint32_t layer);  /* 7*s+1; 0 if layer >= d */
@@ -102,6 +115,9 @@ int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *cuda_stream
 /* fused schedule, builds with -DVC_TRACE only (all zero otherwise): the first n_words <= 65536 trace words of the last
  * launch, each (code << 48 | SM clock of CTA 0) */
 int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, void *cuda_stream);
+/* the device sums of the last vc_verify_transcript_device call on this circuit, n = 4 d + 2 HOST words:
+ * [0] start claim, [1 + 4 i + t] wiring sum of type t of layer i, [1 + 4 d] the input extension at z_d */
+int vc_debug_verifier_sums(const vc_circuit *c, uint64_t *h_sums, uint64_t n);
 /* sticky device-side status: 0 = fine, 1 = a non-canonical input word was seen by vc_evaluate */
 int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */

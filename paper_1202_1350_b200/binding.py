@@ -16,6 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums",
 ]
 
 
@@ -52,6 +53,8 @@ def lib():
             "vc_prove": (i32, [vp, u64, vp, u64, vp]),
             "vc_run_host": (i32, [vp, vp, u64, vp, vp, u64, vp]),
             "vc_verify_transcript": (i32, [vp, vp, vp, u64, vp, u64, vp, vp, vp]),
+            "vc_verify_transcript_device": (i32, [vp, vp, vp, u64, vp, u64, vp, vp, vp, vp]),
+            "vc_debug_verifier_sums": (i32, [vp, vp, u64]),
             "vc_circuit_free": (None, [vp]),
             "vc_strerror": (C.c_char_p, [i32]),
             "vc_transcript_words": (u64, [vp, u32]),
@@ -154,6 +157,21 @@ def vc_verify_transcript(handle: int, h_input, h_outputs, seed: int, h_transcrip
     return bool(acc.value), int(fl.value), int(fr.value)
 
 
+def vc_verify_transcript_device(handle: int, d_input, d_outputs, seed: int, d_transcript, stream=None):
+    """The verifier with its O(S) sums on the GPU; device tensors in, (accept, fail_layer, fail_round) out."""
+    acc, fl, fr = C.c_int(0), C.c_uint32(0), C.c_uint32(0)
+    _check(lib().vc_verify_transcript_device(handle, _dev_ptr(d_input), _dev_ptr(d_outputs), seed, _dev_ptr(d_transcript),
+                                             d_transcript.numel(), C.byref(acc), C.byref(fl), C.byref(fr),
+                                             _stream_ptr(stream)), "vc_verify_transcript_device")
+    return bool(acc.value), int(fl.value), int(fr.value)
+
+
+def vc_debug_verifier_sums(handle: int, d: int) -> np.ndarray:
+    out = np.zeros(4 * d + 2, dtype=np.uint64)
+    _check(lib().vc_debug_verifier_sums(handle, out.ctypes.data, out.size), "vc_debug_verifier_sums")
+    return out
+
+
 def vc_circuit_free(handle: int):
     lib().vc_circuit_free(handle)
 
@@ -226,6 +244,15 @@ class Circuit:
 
     def verify(self, x, outputs, seed, transcript):
         return vc_verify_transcript(self.handle, x, outputs, seed, transcript)
+
+    def verify_device(self, seed: int, d_input=None, d_outputs=None, d_transcript=None, stream=None):
+        """vc_verify_transcript_device on this object's device buffers (or the tensors given)."""
+        return vc_verify_transcript_device(self.handle, self.d_input if d_input is None else d_input,
+                                           self.d_outputs if d_outputs is None else d_outputs, seed,
+                                           self.d_transcript if d_transcript is None else d_transcript, stream)
+
+    def verifier_sums(self) -> np.ndarray:
+        return vc_debug_verifier_sums(self.handle, self.d)
 
     def close(self):
         if self.handle:

@@ -56,6 +56,7 @@ extern "C" const char *vc_strerror(int code) {
 extern "C" void vc_circuit_free(vc_circuit *c) {
     if (!c) return;
     vc::fused_free(c);
+    vc::verifier_free(c);
     for (auto p : c->d_type) cudaFree(p);
     for (auto p : c->d_in1) cudaFree(p);
     for (auto p : c->d_in2) cudaFree(p);

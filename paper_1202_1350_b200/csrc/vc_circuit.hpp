@@ -50,6 +50,7 @@ int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *
 int fused_supported(const vc_circuit *c, uint32_t layer);
 int fused_init(vc_circuit *c);
 void fused_free(const vc_circuit *c);
+void verifier_free(const vc_circuit *c);   // vc_verify_gpu.cu
 int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st);
 int fused_trace(const vc_circuit *c, uint64_t *h, uint32_t n_words, cudaStream_t st);
 int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, cudaStream_t st);

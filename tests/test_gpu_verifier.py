@@ -1,0 +1,140 @@
+"""GPU parity for vc_verify_transcript_device: the verifier's O(S) sums on the device.
+
+Expected values come from oracle/ only: the start claim and the closing input extension are the oracle's MLE, the
+per-type wiring sums are the ones the oracle prover reports per layer (pinned against their definition in
+tests/test_oracle_protocol.py), accept/reject and the failure coordinates are the oracle verifier's.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import vc_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+P = (1 << 61) - 1
+
+
+@pytest.fixture(scope="module")
+def vc():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1202_1350_b200 as v
+    v.lib()
+    return v
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.uint64).view(np.int64)).cuda()
+
+
+def _oracle_sums(c, seed):
+    """[start claim, 4 wiring sums per layer ..., V~_d(z_d)] from the oracle prover, plus its transcript."""
+    oc = oracle.OracleCircuit(c)
+    V = oc.evaluate(c.input)
+    z, claim, ctr = oc.start(V[0], seed)
+    sums, tr = [claim], []
+    for i in range(c.d):
+        t, z, claim, ctr, dbg = oc.prove_layer(i, V[i + 1], seed, ctr, z, claim)
+        tr.append(t)
+        sums += [int(w) for w in dbg.Wsum]
+    sums.append(oracle.mle(c.input, z[:c.log_input]))
+    return np.array(sums, dtype=np.uint64), np.concatenate(tr), V[0]
+
+
+@pytest.mark.parametrize("log_sizes,log_input,seed", [
+    ([1, 2, 3, 2], 3, 61), ([0, 1, 1], 1, 5), ([2, 4, 6, 8, 10, 12], 11, 77), ([0, 11, 12], 13, 21)])
+def test_device_sums_and_verdict_match_oracle(vc, log_sizes, log_input, seed):
+    c = W.random_circuit(log_sizes, log_input, seed)
+    want, tr, out = _oracle_sums(c, 900 + seed)
+    gc = vc.Circuit(c)
+    gc.set_input(c.input)
+    gc.evaluate(); gc.prove(900 + seed)
+    assert np.array_equal(gc.transcript(), tr)
+    assert gc.verify_device(900 + seed) == (True, 0, 0)
+    assert np.array_equal(gc.verifier_sums(), want)                       # every device sum, word for word
+    # the verifier is independent of the prover's buffers: feed it the oracle's transcript and outputs
+    assert gc.verify_device(900 + seed, d_outputs=_dev(out), d_transcript=_dev(tr)) == (True, 0, 0)
+    gc.close()
+
+
+def test_device_verifier_rejects_tampering_like_the_oracle(vc):
+    c = W.random_circuit([1, 2, 3, 2], 3, 61)
+    seed = 808
+    oc = oracle.OracleCircuit(c)
+    out, tr, _, _ = oc.prove(c.input, seed)
+    gc = vc.Circuit(c)
+    d_in, d_out, d_tr = _dev(c.input), _dev(out), _dev(tr)
+    assert gc.verify_device(seed, d_in, d_out, d_tr) == (True, 0, 0)
+    for w in range(tr.size):
+        bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+        got = gc.verify_device(seed, d_in, d_out, _dev(bad))
+        assert got == oc.verify(c.input, out, seed, bad) and not got[0], w
+    for k in range(out.size):
+        bad = out.copy(); bad[k] = (int(bad[k]) + 1) % P
+        assert gc.verify_device(seed, d_in, _dev(bad), d_tr) == oc.verify(c.input, bad, seed, tr) == (False, 0, 0)
+    for k in range(c.input.size):
+        bad = c.input.copy(); bad[k] = (int(bad[k]) + 1) % P
+        assert gc.verify_device(seed, _dev(bad), d_out, d_tr) == oc.verify(bad, out, seed, tr) == (False, c.d, 0)
+    # a wrong seed changes every challenge: the first round check already fails (or, by chance, a later one)
+    assert not gc.verify_device(seed + 1, d_in, d_out, d_tr)[0]
+    gc.close()
+
+
+def test_device_verifier_argument_errors(vc):
+    c = W.random_circuit([1, 2], 2, 3)
+    oc = oracle.OracleCircuit(c)
+    out, tr, _, _ = oc.prove(c.input, 11)
+    gc = vc.Circuit(c)
+    d_in, d_out, d_tr = _dev(c.input), _dev(out), _dev(tr)
+    with pytest.raises(vc.VCError) as e:
+        gc.verify_device(11, d_in, d_out, _dev(tr[:-1]))
+    assert e.value.code == vc.VC_ERR_ARG
+    for which in range(3):                       # a non-canonical word anywhere is an argument error, as on the host
+        bufs = [c.input.copy(), out.copy(), tr.copy()]
+        bufs[which][0] = P
+        with pytest.raises(vc.VCError) as e:
+            gc.verify_device(11, *(_dev(b) for b in bufs))
+        assert e.value.code == vc.VC_ERR_ARG
+    assert gc.verify_device(11, d_in, d_out, d_tr) == (True, 0, 0)
+    gc.close()
+
+
+@pytest.mark.parametrize("k", [1, 2, 4])
+def test_device_verifier_on_configs(vc, k):
+    """Full-size configs in the bench's launch configuration: the honest GPU transcript is accepted, the sums the
+    oracle can compute one by one agree (start claim, closing extension, the widest layer's wiring sums), and a single
+    flipped word is rejected where the host verifier of the library rejects it."""
+    c = W.config(k)
+    seed = W.challenge_seed(k)
+    gc = vc.Circuit(c)
+    gc.set_input(c.input)
+    gc.evaluate(); gc.prove(seed)
+    assert gc.verify_device(seed) == (True, 0, 0)
+    sums = gc.verifier_sums()
+    out, tr = gc.outputs().copy(), gc.transcript().copy()
+    logs = [l.log_size for l in c.layers] + [c.log_input]
+    z0 = [oracle.draw(seed, j) for j in range(logs[0])]
+    assert int(sums[0]) == (oracle.mle(out, z0) if logs[0] else int(out[0]))
+    z, _, _ = gc.state()
+    assert int(sums[-1]) == oracle.mle(c.input, z[:c.log_input])
+    # wiring sums of the widest layer from the oracle's eq tables (Python integers)
+    i = max(range(c.d), key=lambda j: logs[j])
+    zz, _, ctr = oracle.OracleCircuit(c).layer_entry(i, seed, np.zeros(1 << logs[i], dtype=np.uint64))
+    s = logs[i + 1]
+    r1 = [oracle.draw(seed, ctr + j) for j in range(s)]
+    r2 = [oracle.draw(seed, ctr + s + j) for j in range(s)]
+    Tz = oracle.eq_table(zz[:logs[i]]).astype(object)
+    T1 = oracle.eq_table(np.array(r1, dtype=np.uint64)).astype(object)
+    T2 = oracle.eq_table(np.array(r2, dtype=np.uint64)).astype(object)
+    L = c.layers[i]
+    terms = Tz * T1[L.in1] % P * T2[L.in2] % P
+    for t in range(4):
+        assert int(sums[1 + 4 * i + t]) == int(terms[L.type == t].sum() % P), (i, t)
+    rng = np.random.default_rng(k)
+    for w in rng.integers(0, tr.size, size=3):
+        bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+        got = gc.verify_device(seed, d_transcript=_dev(bad))
+        assert got == gc.verify(c.input, out, seed, bad) and not got[0]
+    gc.close()
