@@ -24,8 +24,8 @@ namespace vc {
 using fp61::acc128;
 constexpr int VT = 512;                                   // threads per block of the verifier kernels
 constexpr uint32_t V_EQLOG = 10;                          // eq tables: 2^10 entries for variables 0..9, 2^10 for 10..19
-constexpr size_t V_TAB_WORDS = 2u << V_EQLOG;             // one two-level eq table
-constexpr int V_MAX_BLOCKS = 592;                         // 4 per SM
+constexpr size_t V_TAB_WORDS = (2u << V_EQLOG) + 128;     // one two-level eq table + the four 5-variable factors
+constexpr int V_MAX_BLOCKS = 296;                         // 2 per SM: every block builds its own tables
 
 __device__ __forceinline__ uint64_t warp_sum61(uint64_t v) {  // every lane gets the canonical total
 #pragma unroll
@@ -49,12 +49,22 @@ struct EqTab {
         return e;
     }
 };
-// all threads of the block; the caller synchronises afterwards
-__device__ __forceinline__ EqTab build_eq_tab(uint64_t *tab, const uint64_t *x, uint32_t nv, uint32_t tid) {
-    const uint32_t cl = nv < V_EQLOG ? nv : V_EQLOG, ch = nv < 2 * V_EQLOG ? nv : 2 * V_EQLOG;
+// All threads of the block (one block barrier inside); the caller synchronises afterwards.  Each 2^10-entry half is the
+// outer product of two tables over at most 5 variables (built by direct product in tmp[0..128)): one multiply per entry.
+__device__ __forceinline__ EqTab build_eq_tab(uint64_t *tab, uint64_t *tmp, const uint64_t *x, uint32_t nv, uint32_t tid) {
+    const uint32_t cl = nv < V_EQLOG ? nv : V_EQLOG, ch = nv < 2 * V_EQLOG ? nv : 2 * V_EQLOG, hv = ch - cl;
+    const uint32_t la = cl < 5 ? cl : 5, lb = cl - la, ha = hv < 5 ? hv : 5, hb = hv - ha;
     uint64_t *lo = tab, *hi = tab + (1u << V_EQLOG);
-    for (uint32_t u = tid; u < (1u << cl); u += VT) lo[u] = eq_prod(u, x, 0, cl);
-    for (uint32_t u = tid; u < (1u << (ch - cl)); u += VT) hi[u] = eq_prod(u, x, cl, ch);
+    if (tid < 128) {
+        const uint32_t which = tid >> 5, u = tid & 31;
+        if (which == 0) { if (u < (1u << la)) tmp[u] = eq_prod(u, x, 0, la); }
+        else if (which == 1) { if (u < (1u << lb)) tmp[32 + u] = eq_prod(u, x, la, cl); }
+        else if (which == 2) { if (u < (1u << ha)) tmp[64 + u] = eq_prod(u, x, cl, cl + ha); }
+        else if (u < (1u << hb)) tmp[96 + u] = eq_prod(u, x, cl + ha, ch);
+    }
+    __syncthreads();
+    for (uint32_t u = tid; u < (1u << cl); u += VT) lo[u] = fp61::mul(tmp[u & ((1u << la) - 1)], tmp[32 + (u >> la)]);
+    for (uint32_t u = tid; u < (1u << hv); u += VT) hi[u] = fp61::mul(tmp[64 + (u & ((1u << ha) - 1))], tmp[96 + (u >> ha)]);
     EqTab e; e.lo = lo; e.hi = hi; e.x = x; e.nv = nv;
     return e;
 }
@@ -107,7 +117,7 @@ __global__ void __launch_bounds__(VT) k_v_mle(const uint64_t *__restrict__ V, ui
     const uint32_t tid = threadIdx.x;
     if (tid < s) xs[tid] = x[tid];
     __syncthreads();
-    const EqTab e = build_eq_tab(vsm, xs, s, tid);
+    const EqTab e = build_eq_tab(vsm, vsm + (2u << V_EQLOG), xs, s, tid);
     __syncthreads();
     const uint64_t n = 1ull << s;
     acc128 A; A.clear();
@@ -133,9 +143,9 @@ __global__ void __launch_bounds__(VT) k_v_wiring(const uint8_t *__restrict__ typ
     const uint32_t tid = threadIdx.x;
     if (tid < 3 * MAX_VARS) xs[tid] = pts[tid];
     __syncthreads();
-    const EqTab ez = build_eq_tab(vsm, xs, si, tid);
-    const EqTab e1 = build_eq_tab(vsm + V_TAB_WORDS, xs + MAX_VARS, s, tid);
-    const EqTab e2 = build_eq_tab(vsm + 2 * V_TAB_WORDS, xs + 2 * MAX_VARS, s, tid);
+    const EqTab ez = build_eq_tab(vsm, vsm + (2u << V_EQLOG), xs, si, tid);
+    const EqTab e1 = build_eq_tab(vsm + V_TAB_WORDS, vsm + V_TAB_WORDS + (2u << V_EQLOG), xs + MAX_VARS, s, tid);
+    const EqTab e2 = build_eq_tab(vsm + 2 * V_TAB_WORDS, vsm + 2 * V_TAB_WORDS + (2u << V_EQLOG), xs + 2 * MAX_VARS, s, tid);
     __syncthreads();
     const uint64_t n = 1ull << si;
     acc128 A[4];
@@ -172,7 +182,7 @@ static std::vector<std::pair<const vc_circuit *, VerifierHost>> g_verifiers;
 static VerifierHost *verifier_of(const vc_circuit *c) {
     for (auto &p : g_verifiers) if (p.first == c) return &p.second;
     VerifierHost v;
-    v.blocks = std::min(V_MAX_BLOCKS, 4 * c->sm_count);
+    v.blocks = std::min(V_MAX_BLOCKS, 2 * c->sm_count);
     const size_t npts = (size_t)(c->d + 2) * 3 * MAX_VARS, nres = 4 * (size_t)c->d + 2;
     if (cudaMalloc(&v.d_pts, npts * 8) != cudaSuccess || cudaMalloc(&v.d_res, nres * 8) != cudaSuccess ||
         cudaMalloc(&v.d_part, (size_t)V_MAX_BLOCKS * 4 * 8) != cudaSuccess || cudaMalloc(&v.d_flags, 2 * sizeof(unsigned)) != cudaSuccess ||
@@ -210,18 +220,16 @@ u64 quad_at(const u64 *G, u64 r) {                         // the quadratic thro
     return fp61::add(acc, fp61::mul(G[2], fp61::mul(fp61::mul(r, a), half)));
 }
 u64 power(u64 a, u64 e) { u64 r = 1; for (; e; e >>= 1, a = fp61::mul(a, a)) if (e & 1) r = fp61::mul(r, a); return r; }
-u64 poly_at(const u64 *q, uint32_t s, u64 tau) {           // degree <= s through (k, q[k]), k = 0..s, at tau (barycentric form)
-    if (tau <= s) return q[tau];
-    u64 full = 1, fact = 1;
-    for (uint32_t k = 0; k <= s; k++) full = fp61::mul(full, fp61::sub(tau, k));
-    for (uint32_t k = 2; k <= s; k++) fact = fp61::mul(fact, k);
-    std::vector<u64> invf(s + 1);
-    u64 inv = power(fact, fp61::P - 2);
-    for (int k = (int)s; k >= 0; k--) { invf[k] = inv; inv = fp61::mul(inv, (u64)(k ? k : 1)); }
+// degree <= s through (k, q[k]), k = 0..s, at tau: sum_k q[k] prod_{m != k}(tau - m) / (k! (s-k)! (-1)^(s-k)); the products
+// come from prefix and suffix tables, invf[k] = 1/k! from one inversion per call of the verifier
+u64 poly_at(const u64 *q, uint32_t s, u64 tau, const std::vector<u64> &invf) {
+    std::vector<u64> pre(s + 2), suf(s + 2);
+    pre[0] = 1; suf[s + 1] = 1;
+    for (uint32_t k = 0; k <= s; k++) pre[k + 1] = fp61::mul(pre[k], fp61::sub(tau, k));
+    for (uint32_t k = s + 1; k-- > 0;) suf[k] = fp61::mul(suf[k + 1], fp61::sub(tau, k));
     u64 tot = 0;
     for (uint32_t k = 0; k <= s; k++) {
-        // weight_k = 1 / (k! (s-k)! (-1)^(s-k)),  term = q[k] weight_k full / (tau - k)
-        u64 t = fp61::mul(fp61::mul(q[k], fp61::mul(invf[k], invf[s - k])), fp61::mul(full, power(fp61::sub(tau, k), fp61::P - 2)));
+        const u64 t = fp61::mul(fp61::mul(q[k], fp61::mul(pre[k], suf[k + 1])), fp61::mul(invf[k], invf[s - k]));
         tot = ((s - k) & 1) ? fp61::sub(tot, t) : fp61::add(tot, t);
     }
     return tot;
@@ -278,6 +286,16 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
     if (h_flags[1]) return VC_ERR_ARG;                         // non-canonical input or output word
     for (u64 w = 0; w < n_words; w++) if (h_tr[w] >= fp61::P) return VC_ERR_ARG;
     // ---- the O(rounds) checks, in protocol order
+    uint32_t smax = 1;
+    for (uint32_t i = 1; i <= d; i++) smax = std::max(smax, c->logs[i]);
+    std::vector<u64> invf(smax + 1);
+    {
+        u64 fact = 1;
+        for (uint32_t k = 2; k <= smax; k++) fact = fp61::mul(fact, k);
+        u64 inv = power(fact, fp61::P - 2);
+        for (uint32_t k = smax; k >= 1; k--) { invf[k] = inv; inv = fp61::mul(inv, k); }
+        invf[0] = 1;
+    }
     u64 claim = h_res[0];
     const u64 *tr = h_tr;
     for (uint32_t i = 0; i < d; i++) {
@@ -292,7 +310,7 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
         u64 rhs = 0;
         for (uint32_t t = 0; t < 4; t++) rhs = fp61::add(rhs, fp61::mul(W[t], apply_gate(t, q[0], q[1])));
         if (rhs != claim) { *fail_layer = i; *fail_round = 2 * s; return VC_OK; }
-        claim = poly_at(q, s, taus[i]);
+        claim = poly_at(q, s, taus[i], invf);
     }
     if (h_res[1 + 4 * (size_t)d] != claim) { *fail_layer = d; *fail_round = 0; return VC_OK; }
     *accept = 1;
