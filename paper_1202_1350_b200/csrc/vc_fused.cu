@@ -16,6 +16,9 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     uint32_t *pas = reinterpret_cast<uint32_t *>(smem + F_PASCAL_OFF);             // C(n,k), n,k < 32
     uint8_t *dyn = smem + F_FIXED_BYTES;
     const uint32_t tid = threadIdx.x;
+#ifdef VC_TRACE
+    if (tid == 0) { g_tr_stamps = a.stamps; g_tr_d = a.d; }
+#endif
     // ---- load (or start) the proof state
     if (a.begin == 0) {
         const uint32_t s0 = a.L[0].log_n;

@@ -94,8 +94,18 @@ constexpr uint32_t F_TRACE_WORDS = 1u << 16;
             cx.pad++;                                                                                        \
         }                                                                                                    \
     } while (0)
+static __device__ uint64_t *g_tr_stamps;
+static __device__ uint32_t g_tr_d;
+#define VC_TRL(code)                                                                                         \
+    do {                                                                                                     \
+        if (blockIdx.x == 0 && threadIdx.x == 0 && cx.pad < F_TRACE_WORDS) {                                 \
+            g_tr_stamps[g_tr_d + 1 + cx.pad] = ((uint64_t)(code) << 48) | ((uint64_t)clock64() & 0xffffffffffffull); \
+            cx.pad++;                                                                                        \
+        }                                                                                                    \
+    } while (0)
 #else
 #define VC_TR(code) do { } while (0)
+#define VC_TRL(code) do { } while (0)
 #endif
 
 __device__ __forceinline__ uint64_t fold2(uint64_t a, uint64_t b, uint64_t r) {

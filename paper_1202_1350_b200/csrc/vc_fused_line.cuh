@@ -7,8 +7,9 @@
 // multiplies; the extra node of each lower level comes from its finite differences) and continues it to P = tb + 4
 // nodes t = 0..P-1 with three additions per node.  The block of 2^tb threads then folds variables 3..3+tb-1 in shared
 // memory, one multiply per (node, t): about P multiplies per thread in all, instead of (s-1) multiply + warp-reduce
-// steps.  The block's polynomial (degree <= P-1, known at P nodes) is continued to t = P..s by Newton's forward
-// differences with binomial coefficients, weighted with eq(block bits, l(t)) and accumulated.
+// steps.  The block's polynomial (degree <= P-1, known at P nodes) is continued to t = P..s by Lagrange interpolation on
+// the integer nodes (integer coefficients from Pascal's triangle, 16 lanes per t), weighted with eq(block bits, l(t))
+// and accumulated.
 #pragma once
 #include "vc_fused.cuh"
 
@@ -55,10 +56,16 @@ __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, Fused
     uint64_t *B = A + (size_t)NB * P;
     uint64_t *fx = B + (((size_t)NB * P + 1) / 2 + 1 & ~(size_t)1);
     uint64_t *dl = fx + 32;
+    VC_TRL(70);
     for (uint32_t i = tid; i < m; i += nthr) cx.acc[i] = 0;
-    for (uint32_t i = tid; i < (s + 1) * sp; i += nthr) {
-        const uint32_t t = i / sp, k = i % sp;
-        pts[i] = k < s ? fp61::add(cx.r1[k], fp61::mul(t, fp61::sub(cx.r2[k], cx.r1[k]))) : 0;
+    {   // lane k of every warp owns variable k (sp <= 30); warp w takes t = w, w + nw, ...: l(t + nw) = l(t) + nw d, no division
+        const uint32_t lane = tid & 31, w = tid >> 5, nw = nthr >> 5;
+        if (lane < sp) {
+            const uint64_t p = lane < s ? cx.r1[lane] : 0, q = lane < s ? cx.r2[lane] : 0, d = fp61::sub(q, p);
+            const uint64_t step = nw == 1 ? d : fp61::mul(nw, d);
+            uint64_t v = w == 0 ? p : fp61::add(p, fp61::mul(w, d));
+            for (uint32_t t = w; t <= s; t += nw) { pts[t * sp + lane] = v; v = fp61::add(v, step); }
+        }
     }
     // l(t)_k for k < 3 at t = 0..3
     uint64_t x[3][4];
@@ -67,6 +74,7 @@ __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, Fused
         const uint64_t p = (uint32_t)k < s ? cx.r1[k] : 0, q = (uint32_t)k < s ? cx.r2[k] : 0, d = fp61::sub(q, p);
         x[k][0] = p; x[k][1] = q; x[k][2] = fp61::add(q, d); x[k][3] = fp61::add(x[k][2], d);
     }
+    VC_TRL(71);
     for (uint32_t vb = vb0; vb < nvb; vb += vbstride) {
         if (tid < NB) {
             uint64_t v[8];
@@ -114,7 +122,9 @@ __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, Fused
                 A[(size_t)t * NB + tid] = cur;
             }
         }
+        VC_TRL(72);
         bar_n(nthr);                                             // also publishes pts on the first pass
+        VC_TRL(73);
         // the block's fold tree over variables 3..3+tb-1: level lev halves the nodes, one multiply per (node, t)
         uint64_t *in = A, *out = B;
         for (uint32_t lev = 0; lev < tb; lev++) {
@@ -127,35 +137,36 @@ __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, Fused
             bar_n(nthr);
             uint64_t *tmp = in; in = out; out = tmp;
         }
-        // in[pt], pt < P: the block polynomial.  Continue it to t = P..s (Newton forward differences).
+        VC_TRL(74);
+        // in[pt], pt < P: the block polynomial.  Continue it to t = P..s.
         if (s + 1 > P) {
-            if (tid < P) {                                       // dl[k] = sum_i (-1)^(k-i) C(k,i) f(i)
-                acc128 pos, neg; pos.clear(); neg.clear();
-                for (uint32_t i = 0; i <= tid; i++) {
-                    const uint64_t cki = pas[tid * 32 + i];
-                    if ((tid - i) & 1u) neg.mac(cki, in[i]); else pos.mac(cki, in[i]);
+            // Lagrange on the integer nodes 0..P-1 at an integer t >= P:  f(t) = sum_i (-1)^(P-1-i) C(t,i) C(t-1-i, P-1-i) f(i)
+            // (prod_{m != i}(t - m) / prod_{m != i}(i - m), an integer below 2^54 for t <= 30).  Sixteen lanes per t (P <= 13),
+            // one multiply per lane, four shuffle steps: no serial pass over the nodes.
+            if (tid < P) fx[tid] = in[tid];
+            const uint32_t nit = (s + 1 - P) * 16;
+            for (uint32_t base = 0; base < nit; base += nthr) {
+                const uint32_t item = base + tid, t = P + (item >> 4), i = item & 15;
+                uint64_t term = 0;
+                if (item < nit && i < P) {
+                    const uint64_t coef = (uint64_t)pas[t * 32 + i] * pas[(t - 1 - i) * 32 + (P - 1 - i)];
+                    term = fp61::mul(coef, in[i]);
+                    if ((P - 1 - i) & 1u) term = fp61::neg(term);
                 }
-                dl[tid] = fp61::sub(pos.value(), neg.value());
-            }
-            bar_n(nthr);
-            if (tid <= s) {
-                uint64_t val;
-                if (tid < P) val = in[tid];
-                else {                                           // f(t) = sum_k C(t,k) dl[k]
-                    acc128 a; a.clear();
-                    for (uint32_t k = 0; k < P; k++) a.mac(pas[tid * 32 + k], dl[k]);
-                    val = a.value();
-                }
-                fx[tid] = val;
+#pragma unroll
+                for (int off = 8; off; off >>= 1) term = fp61::add(term, __shfl_xor_sync(0xffffffffu, term, off));
+                if (item < nit && i == 0) fx[t] = term;
             }
         } else if (tid <= s) {
             fx[tid] = in[tid];
         }
         bar_n(nthr);
+        VC_TRL(75);
         if (tid >= 2 && tid <= s) {
             const uint64_t e = eq_direct(vb, pts + (size_t)tid * sp, 3 + tb, sp);     // eq(block bits, l(t))
             cx.acc[tid - 2] = fp61::add(cx.acc[tid - 2], fp61::mul(fx[tid], e));
         }
+        VC_TRL(76);
         bar_n(nthr);
     }
     if (vb0 >= nvb) bar_n(nthr);                                 // pts / acc settled even without a block
@@ -168,17 +179,22 @@ __device__ __noinline__ void line_finish(uint32_t s, FusedCtx &cx, const uint64_
     if (tid >= 32) return;
     const uint32_t k = tid;
     const uint64_t tau = fp61::draw(cx.seed, cx.ctr);
+    // prod_{mm != k} (tau - mm) for every lane k at once: prefix and suffix products of the factors across the warp
+    // (five shuffle + multiply steps each, interleaved), instead of one serial pass over the nodes per lane
+    const uint64_t f = k <= s ? fp61::sub(tau, k) : 1;
+    uint64_t pre = f, suf = f;
+#pragma unroll
+    for (uint32_t off = 1; off < 32; off <<= 1) {
+        const uint64_t up = __shfl_up_sync(0xffffffffu, pre, off), dn = __shfl_down_sync(0xffffffffu, suf, off);
+        if (k >= off) pre = fp61::mul(pre, up);
+        if (k + off < 32) suf = fp61::mul(suf, dn);
+    }
+    const uint64_t pl = __shfl_up_sync(0xffffffffu, pre, 1), sr = __shfl_down_sync(0xffffffffu, suf, 1);
     uint64_t term = 0;
     if (k <= s) {
         const uint64_t qk = k == 0 ? cx.v1 : (k == 1 ? cx.v2 : cx.acc[k - 2]);
         if (writer) tr_q[k] = qk;
-        uint64_t c[4] = {1, 1, 1, 1};                          // prod_{mm != k} (tau - mm), four interleaved chains
-        for (uint32_t mm = 0; mm <= s; mm += 4) {
-#pragma unroll
-            for (uint32_t e = 0; e < 4; e++)
-                if (mm + e <= s && mm + e != k) c[e] = fp61::mul(c[e], fp61::sub(tau, mm + e));
-        }
-        const uint64_t num = fp61::mul(fp61::mul(c[0], c[1]), fp61::mul(c[2], c[3]));
+        const uint64_t num = fp61::mul(k ? pl : 1, k < 31 ? sr : 1);
         const uint64_t dinv = fp61::mul(invfact[k], invfact[s - k]);
         term = fp61::mul(qk, fp61::mul(num, dinv));
         if ((s - k) & 1u) term = fp61::neg(term);
