@@ -36,14 +36,16 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
 
     // ---- a3 + phase-1 state
     __syncthreads();
+    VC_TR(30);
     uint32_t ctr = (uint32_t)cx.ctr;
     const EqTab eb = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);
     __syncthreads();
+    VC_TR(31);
     uint32_t i1 = 0, i2 = 0, t = VC_RELAY, idx = 0;
-    uint64_t W = 0, cP = fp61::P;
+    uint64_t W = 0, cP = fp61::P, P = 0;             // P: the plain weight beta(z,g) eq(low bits of in1[g], r1[0..j)), tracked in phase 1
     if (live) {
         i1 = __ldg(Lp.in1 + g); i2 = __ldg(Lp.in2 + g); t = __ldg(Lp.type + g);
-        const uint64_t P = eb.eq_of(g);
+        P = eb.eq_of(g);
         uint64_t c; uint32_t ign;
         gate_state(1, t, P, __ldg(Vb + i2), W, c, ign);
         cP = c + fp61::P; idx = i1;
@@ -57,26 +59,26 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
         grid_allreduce(cx, a, 1, false);
         if (tid == 0) cx.claim = cx.acc[0];
     }
+    VC_TR(32);
     __syncthreads();
+    VC_TR(33);
     uint32_t ep = cx.epoch, par = 0;
     RoundPend pd; pd.tr1 = pd.tr2 = nullptr; pd.s1 = pd.s2 = 0;
 
     for (int ph = 0; ph < 2; ph++) {
         const uint32_t K = Lp.K[ph], blo = cp.blo[ph], nbk = cp.nb[ph];
         uint64_t *rr = ph == 0 ? cx.r1 : cx.r2;
-        if (ph == 1) {                               // phase switch: P = beta(z,g) eq(in1[g], r1), then the phase-2 state
-            __syncthreads();
-            const uint64_t v1 = cx.v1;
-            const EqTab e0 = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);
-            const EqTab e1 = build_eq_tab(bufX + (2u << F_EQLOG), bufX + (3u << F_EQLOG), scr + 128, cx.r1, s, tid, FT);
-            __syncthreads();
+        if (ph == 1) {                               // phase switch: P = beta(z,g) eq(in1[g], r1) is in the register; the phase-2 state
+            VC_TR(34);
+            __syncthreads();                         // v1 and r1[s-1] are visible
+            VC_TR(35);
             if (live) {
-                const uint64_t P = fp61::mul(e0.eq_of(g), e1.eq_of(i1));
+                P = fp61::mul(P, ((i1 >> (s - 1)) & 1u) ? cx.r1[s - 1] : fp61::sub(1, cx.r1[s - 1]));   // the last factor of phase 1
                 uint64_t c; uint32_t ign;
-                gate_state(2, t, P, v1, W, c, ign);
+                gate_state(2, t, P, cx.v1, W, c, ign);
                 cP = c + fp61::P; idx = i2 | (ign << 31);
             }
-            __syncthreads();
+            VC_TR(37);
         }
         uint64_t r_prev = 0;
         for (uint32_t j = 0; j < s; j++) {
@@ -108,7 +110,9 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
                         q1 = *reinterpret_cast<const ulonglong2 *>(src + (4 * (size_t)u - base) + 2);
                     }
                     lo = fold2(q0.x, q0.y, r_prev); hi = fold2(q1.x, q1.y, r_prev);
-                    W = fp61::mul(W, ((idx >> (j - 1)) & 1u) ? r_prev : fp61::sub(1, r_prev));
+                    const uint64_t fj = ((idx >> (j - 1)) & 1u) ? r_prev : fp61::sub(1, r_prev);
+                    W = fp61::mul(W, fj);
+                    if (ph == 0) P = fp61::mul(P, fj);   // off the products' chain: spares two eq tables at the phase switch
                 }
                 if (has_ign && (idx >> 31)) { lo = 0; hi = 0; }
                 const uint64_t mb = (bit ? hi : lo) + cP, m2 = 2 * hi + cP - lo;
@@ -170,15 +174,16 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
         }
     }
     if (tid == 0) { cx.ctr = ctr; cx.epoch = ep; }
-    if (warp == 15) reducer_flush(a, pd);
     __syncthreads();
     VC_TR(17);
-    // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
+    // ---- a7: line restriction, all CTAs share the pass over V_{i+1}; the reducer converts the last two rounds'
+    // messages into transcript words beside it (their slots are not touched by the all-reduce below: ring of 8)
     if (s > 1) {
         const uint32_t ltb = fused_line_tb_grid(s, FT), lthr = (1u << ltb) > 32 ? (1u << ltb) : 32;
         if (tid < lthr) line_partials(Vb, s, cx, pas, reinterpret_cast<uint64_t *>(dyn), b, G, tid, lthr, ltb);
+        if (warp == 15) reducer_flush(a, pd);        // lthr <= 2^7 on this path: warp 15 is never in line_partials
         grid_allreduce(cx, a, s - 1, false);
-    }
+    } else if (warp == 15) reducer_flush(a, pd);
     VC_TR(18);
     line_finish(s, cx, invfact, tr, b == 0, tid);
     __syncthreads();
