@@ -176,9 +176,14 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     k = args.config
     c = W.config(k)
-    if args.f2_log_n:                            # paper-scale F2: same construction as config 2, n = 2^f2_log_n
+    if args.f2_log_n and not args.paper_scale:
+        args.paper_scale = f"f2:{args.f2_log_n}"
+    if args.paper_scale:                         # paper-scale workloads: the constructions of configs 2-5 at Table 2's sizes
         from vc_workloads import circuits
-        c = circuits.f2_circuit(args.f2_log_n, W.data_seed(2))
+        kind, n = args.paper_scale.split(":")
+        n = int(n)
+        c = {"f2": lambda: circuits.f2_circuit(n, W.data_seed(2)), "f0": lambda: circuits.f0_circuit(n, W.data_seed(3)),
+             "matmul": lambda: circuits.matmul_circuit(n, W.data_seed(4)), "pm": lambda: circuits.pm_circuit(n, 3, W.data_seed(5))}[kind]()
         k = 0
     from paper_1202_1350_b200 import replicas
     c.input = replicas.replica_input(c.input, W.data_seed(k or 2), rank)   # replicas: same circuit, another seeded input
@@ -353,6 +358,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
     args = ap.parse_args()
     if args.impl == "reference":
