@@ -64,7 +64,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                 __syncthreads();
                 handoff = false;
             }
-            if (a.L[layer].thin) thin_layer(a, cx, invfact, pas, dyn, layer, tr);
+            if (a.L[layer].thin == 4) thin_layer<4>(a, cx, invfact, pas, dyn, layer, tr);
+            else if (a.L[layer].thin) thin_layer<1>(a, cx, invfact, pas, dyn, layer, tr);
             else wide_layer(a, cx, invfact, pas, dyn, layer, tr);
         }
         tr += 7 * (size_t)s + 1;
@@ -197,7 +198,8 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         const size_t total = std::max(F_FIXED_BYTES + F_THIN_COMMIT_BYTES + tabw * 8 + scr_words * 8,
                                       F_FIXED_BYTES + fused_line_words(s, FT) * 8);
         if (total <= F_SMEM_MAX) {
-            lp.thin = 1; lp.cap = (uint32_t)cap;
+            lp.thin = ngmax <= F_WORKERS / 4 ? 4 : 1;        // lanes per gate
+            lp.cap = (uint32_t)cap;
             for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = F_MODE_SLICE; lp.K[ph] = K; }
             lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
             lp.off_tab = (uint32_t)F_THIN_COMMIT_BYTES;

@@ -45,7 +45,7 @@ struct LayerPlan {
     const CtaPlan *cta;                  // gridDim entries (wide layers), else null
     uint32_t log_n;
     uint32_t kind;                       // 0: single CTA, 1: grid-wide
-    uint32_t thin;                       // 1: at most one gate per worker thread: vc_fused_thin.cuh
+    uint32_t thin;                       // != 0: at most one gate per worker thread: vc_fused_thin.cuh; the value = lanes per gate (1 or 4)
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
     uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
     uint32_t cap;                        // state capacity in gates (multiple of FT)

@@ -18,6 +18,13 @@ namespace vc {
 
 constexpr size_t F_THIN_COMMIT_BYTES = 2 * (size_t)FT * 16;
 
+// LPG = lanes per gate (1 or 4).  With at most F_WORKERS / 4 gates per CTA a gate is spread over four neighbouring lanes: after the
+// challenge arrives each lane does ONE of the four multiplies that depend on it (fold lo, fold hi, W update, P update),
+// the results are exchanged by shuffles, and lanes 0 and 1 do one product each — the chain from challenge to commit
+// is two multiplies deep on every lane instead of five multiplies issued by one.  All lanes run the same instruction
+// stream (operands are selected, not branched on); gates beyond ng mirror the last gate and commit nothing.  (Two lanes per gate
+// for up to F_WORKERS / 2 gates was measured and is slower than one: 71.3 against 67.2 us on config 2's layer 15.)
+template <int LPG>
 __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas,
                                            uint8_t *dyn, uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x, b = blockIdx.x;
@@ -27,8 +34,11 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
     const uint64_t *__restrict__ Vb = a.L[layer + 1].V;
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;           // ng <= F_WORKERS
-    const bool live = tid < ng;
-    const uint32_t g = live ? g0 + tid : g0;
+    const uint32_t q = LPG == 1 ? 0 : tid & (LPG - 1), gi = LPG == 4 ? tid >> 2 : tid;
+    const bool live = gi < ng;                               // this lane's gate exists
+    constexpr uint32_t GPW = 32 / LPG;                       // gates per warp
+    const bool act = LPG == 1 ? live : gi < ((ng + GPW - 1) & ~(GPW - 1));   // uniform within a warp for LPG > 1
+    const uint32_t g = g0 + (live ? gi : (ng ? ng - 1 : 0));
     ulonglong2 *cbuf = reinterpret_cast<ulonglong2 *>(dyn);   // [2][FT] committed products
     uint64_t *bufX = reinterpret_cast<uint64_t *>(dyn + Lp.off_tab), *bufY = bufX + Lp.xw;
     uint64_t *scr = reinterpret_cast<uint64_t *>(dyn + Lp.off_scr);
@@ -43,7 +53,7 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
     VC_TR(31);
     uint32_t i1 = 0, i2 = 0, t = VC_RELAY, idx = 0;
     uint64_t W = 0, cP = fp61::P, P = 0;             // P: the plain weight beta(z,g) eq(low bits of in1[g], r1[0..j)), tracked in phase 1
-    if (live) {
+    if (act) {
         i1 = __ldg(Lp.in1 + g); i2 = __ldg(Lp.in2 + g); t = __ldg(Lp.type + g);
         P = eb.eq_of(g);
         uint64_t c; uint32_t ign;
@@ -51,7 +61,7 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
         cP = c + fp61::P; idx = i1;
     }
     if (layer == 0) {                                // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
-        uint64_t part = live ? fp61::mul(eb.eq_of(g), __ldg(Lp.V + g)) : 0;
+        uint64_t part = (live && q == 0) ? fp61::mul(eb.eq_of(g), __ldg(Lp.V + g)) : 0;
         part = warp_sum61(part);
         if (lane == 0) cx.red[warp * 4] = part;
         __syncthreads();
@@ -72,7 +82,7 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
             VC_TR(34);
             __syncthreads();                         // v1 and r1[s-1] are visible
             VC_TR(35);
-            if (live) {
+            if (act) {
                 P = fp61::mul(P, ((i1 >> (s - 1)) & 1u) ? cx.r1[s - 1] : fp61::sub(1, cx.r1[s - 1]));   // the last factor of phase 1
                 uint64_t c; uint32_t ign;
                 gate_state(2, t, P, cx.v1, W, c, ign);
@@ -89,7 +99,7 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
                 fence = true;
             }
             // ---- a4 for this thread's gate, against level j-1 folded on the fly (level 0 in round 0)
-            if (live) {
+            if (act) {
                 const uint32_t bit = (idx >> j) & 1u, u = (idx & F_IDX_MASK) >> (j + 1);
                 uint64_t lo, hi;
                 if (j == 0) {
@@ -109,17 +119,35 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
                         q0 = *reinterpret_cast<const ulonglong2 *>(src + (4 * (size_t)u - base));
                         q1 = *reinterpret_cast<const ulonglong2 *>(src + (4 * (size_t)u - base) + 2);
                     }
-                    lo = fold2(q0.x, q0.y, r_prev); hi = fold2(q1.x, q1.y, r_prev);
                     const uint64_t fj = ((idx >> (j - 1)) & 1u) ? r_prev : fp61::sub(1, r_prev);
-                    W = fp61::mul(W, fj);
-                    if (ph == 0) P = fp61::mul(P, fj);   // off the products' chain: spares two eq tables at the phase switch
+                    if (LPG == 4) {
+                        // lane 0: lo = x0 + r (x1 - x0) of the first pair, lane 1: hi of the second, lane 2: W fj, lane 3: P fj
+                        const uint64_t x0 = q == 0 ? q0.x : q1.x, x1 = q == 0 ? q0.y : q1.y;
+                        const uint64_t ma = q < 2 ? r_prev : (q == 2 ? W : P), mb_ = q < 2 ? fp61::sub(x1, x0) : fj;
+                        const uint64_t pr = fp61::mul(ma, mb_), val = q < 2 ? fp61::add(x0, pr) : pr;
+                        const uint32_t l4 = lane & ~3u;
+                        lo = __shfl_sync(0xffffffffu, val, l4); hi = __shfl_sync(0xffffffffu, val, l4 + 1);
+                        W = __shfl_sync(0xffffffffu, val, l4 + 2);
+                        const uint64_t Pn = __shfl_sync(0xffffffffu, val, l4 + 3);
+                        if (ph == 0) P = Pn;
+                    } else {
+                        lo = fold2(q0.x, q0.y, r_prev); hi = fold2(q1.x, q1.y, r_prev);
+                        W = fp61::mul(W, fj);
+                        if (ph == 0) P = fp61::mul(P, fj);   // off the products' chain: spares two eq tables at the phase switch
+                    }
                 }
                 if (has_ign && (idx >> 31)) { lo = 0; hi = 0; }
                 const uint64_t mb = (bit ? hi : lo) + cP, m2 = 2 * hi + cP - lo;
-                ulonglong2 o;
-                o.x = fp61::fold128(fp61::mulhi(W, mb), W * mb) | ((uint64_t)bit << 63);
-                o.y = fp61::fold128(fp61::mulhi(W, m2), W * m2);
-                cbuf[par * FT + tid] = o;
+                if (LPG > 1) {                       // lane 0: W (x_b + c) with the bit, lane 1: W (x_2 + c)
+                    const uint64_t m = q == 0 ? mb : m2;
+                    const uint64_t pr = fp61::fold128(fp61::mulhi(W, m), W * m) | (q == 0 ? (uint64_t)bit << 63 : 0);
+                    if (live && q < 2) reinterpret_cast<uint64_t *>(cbuf + par * FT + gi)[q] = pr;
+                } else {
+                    ulonglong2 o;
+                    o.x = fp61::fold128(fp61::mulhi(W, mb), W * mb) | ((uint64_t)bit << 63);
+                    o.y = fp61::fold128(fp61::mulhi(W, m2), W * m2);
+                    cbuf[par * FT + tid] = o;
+                }
             }
             VC_TR(41);
             __syncthreads();                         // every contribution of this CTA to message j is committed
