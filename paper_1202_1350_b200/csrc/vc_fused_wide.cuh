@@ -24,6 +24,17 @@ __device__ __noinline__ void publish_level(const uint64_t *__restrict__ Vb, cons
                                               uint32_t e1, uint64_t *eqt, uint64_t *Tg) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     __syncthreads();                                             // rr[km1-1] (written by the last rendezvous) is visible
+    if (km1 <= 5) {                                              // 2^km1 lanes per entry: no table, no further barrier
+        const uint32_t gs = 1u << km1, per = 32u >> km1, sub = lane & (gs - 1), ent = lane >> km1;
+        const uint64_t w = eq_direct(sub, rr, 0, km1);
+        for (uint32_t ew = e0 + warp * per; ew < e1; ew += (FT / 32) * per) {
+            const uint32_t e = ew + ent;
+            uint64_t v = e < e1 ? fp61::mul(w, __ldg(Vb + ((size_t)e << km1) + sub)) : 0;
+            for (uint32_t off = gs >> 1; off; off >>= 1) v = fp61::add(v, __shfl_xor_sync(0xffffffffu, v, off));
+            if (sub == 0 && e < e1) __stcg(Tg + e, v);
+        }
+        return;
+    }
     build_eq10(eqt + 64, eqt, rr, 0, km1, tid, FT);              // eqt[0..64): the two 5-variable factors
     __syncthreads();
     eqt += 64;
