@@ -48,16 +48,20 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
     __syncthreads();
     VC_TR(30);
     uint32_t ctr = (uint32_t)cx.ctr;
+    uint32_t i1 = 0, i2 = 0, t = VC_RELAY, idx = 0;
+    uint64_t W = 0, cP = fp61::P, P = 0;             // P: the plain weight beta(z,g) eq(low bits of in1[g], r1[0..j)), tracked in phase 1
+    uint64_t other = 0;
+    if (act) {                                       // the gate's record and fixed operand travel while the eq table is built
+        i1 = __ldg(Lp.in1 + g); i2 = __ldg(Lp.in2 + g); t = __ldg(Lp.type + g);
+        other = __ldg(Vb + i2);
+    }
     const EqTab eb = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);
     __syncthreads();
     VC_TR(31);
-    uint32_t i1 = 0, i2 = 0, t = VC_RELAY, idx = 0;
-    uint64_t W = 0, cP = fp61::P, P = 0;             // P: the plain weight beta(z,g) eq(low bits of in1[g], r1[0..j)), tracked in phase 1
     if (act) {
-        i1 = __ldg(Lp.in1 + g); i2 = __ldg(Lp.in2 + g); t = __ldg(Lp.type + g);
         P = eb.eq_of(g);
         uint64_t c; uint32_t ign;
-        gate_state(1, t, P, __ldg(Vb + i2), W, c, ign);
+        gate_state(1, t, P, other, W, c, ign);
         cP = c + fp61::P; idx = i1;
     }
     if (layer == 0) {                                // a2: start claim V~_0(z_0) = sum_g beta(z_0,g) V_0[g]
