@@ -80,7 +80,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
 
 // ---- a1 in one launch: V_d <- input (checked canonical), then V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]) for
 // i = d-1..0 (all gates of a layer in parallel, layer after layer).  Grid-wide layers are separated by a
-// counter rendezvous; once the remaining layers are narrow CTA 0 finishes them alone behind block barriers.
+// counter rendezvous; once the remaining layers are narrow CTA 0 finishes them alone behind block barriers, with the
+// values in shared memory and the next layer's records fetched ahead.
 constexpr int EVAL_T = 1024;
 constexpr uint32_t EVAL_NARROW_LOG = 11;
 __device__ __forceinline__ void eval_grid_barrier(unsigned long long *cnt, uint32_t &gen) {
@@ -109,24 +110,63 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
         }
         if (bad) atomicOr(&st->flags, 1u);
     }
-    bool solo = false;                            // CTA 0 alone from the first layer whose inputs and outputs are narrow
-    for (int i = (int)d - 1; i >= 0; i--) {
+    extern __shared__ __align__(16) uint64_t ev_sm[];   // the narrow tail: two value tables of 2^(EVAL_NARROW_LOG+1) words
+    int i = (int)d - 1;
+    for (; i >= 0; i--) {                         // grid-wide layers, separated by a counter rendezvous
+        if (L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1) break;
         const uint32_t n = 1u << L[i].log_n;
-        const bool narrow = L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1;
-        if (!solo) eval_grid_barrier(cnt, gen); else __syncthreads();
-        if (narrow && !solo) { solo = true; if (b != 0) return; }
         const uint8_t *__restrict__ type = L[i].type;
         const uint32_t *__restrict__ in1 = L[i].in1, *__restrict__ in2 = L[i].in2;
         const uint64_t *Vb = L[i + 1].V;
         uint64_t *Vo = const_cast<uint64_t *>(L[i].V);
-        const uint32_t start = solo ? tid : b * EVAL_T + tid, stride = solo ? EVAL_T : G * EVAL_T;
-        for (uint32_t g = start; g < n; g += stride) {
+        eval_grid_barrier(cnt, gen);
+        for (uint32_t g = b * EVAL_T + tid; g < n; g += G * EVAL_T) {
             const uint64_t v = gate_f(type[g], __ldcg(Vb + in1[g]), __ldcg(Vb + in2[g]));
             Vo[g] = v;
             if (i == 0 && out0) out0[g] = v;
         }
     }
+    if (i < 0) return;
+    // ---- CTA 0 finishes the narrow layers alone: values ping-pong in shared memory (every V_i is still written out
+    // for the prover), and the records of the next layer are fetched before the barrier that ends the current one
+    eval_grid_barrier(cnt, gen);
+    if (b != 0) return;
+    constexpr uint32_t TW = 2u << EVAL_NARROW_LOG, NG = (1u << EVAL_NARROW_LOG) / EVAL_T;   // table words; gates per thread
+    uint64_t *cur = ev_sm, *nxt = ev_sm + TW;
+    {
+        const uint64_t *Vb = L[i + 1].V;
+        for (uint32_t u = tid; u < (1u << L[i + 1].log_n); u += EVAL_T) cur[u] = __ldcg(Vb + u);
+    }
+    uint32_t rt[NG], ra[NG], rb[NG];
+    auto fetch = [&](int layer) {
+        const uint32_t n = 1u << L[layer].log_n;
+#pragma unroll
+        for (uint32_t k = 0; k < NG; k++) {
+            const uint32_t g = k * EVAL_T + tid;
+            if (g < n) { rt[k] = __ldg(L[layer].type + g); ra[k] = __ldg(L[layer].in1 + g); rb[k] = __ldg(L[layer].in2 + g); }
+        }
+    };
+    fetch(i);
+    __syncthreads();
+    for (; i >= 0; i--) {
+        const uint32_t n = 1u << L[i].log_n;
+        uint64_t *Vo = const_cast<uint64_t *>(L[i].V);
+#pragma unroll
+        for (uint32_t k = 0; k < NG; k++) {
+            const uint32_t g = k * EVAL_T + tid;
+            if (g < n) {
+                const uint64_t v = gate_f(rt[k], cur[ra[k]], cur[rb[k]]);
+                nxt[g] = v; Vo[g] = v;
+                if (i == 0 && out0) out0[g] = v;
+            }
+        }
+        if (i > 0) fetch(i - 1);
+        __syncthreads();
+        uint64_t *t = cur; cur = nxt; nxt = t;
+    }
 }
+
+constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
 
@@ -282,7 +322,8 @@ int fused_init(vc_circuit *c) {
     if (cudaMalloc(&fh.d_evcnt, 64) != cudaSuccess) return VC_ERR_NOMEM;
     {   // the one-launch evaluation needs: a co-resident grid, and narrow layers only at the output end
         int eper = 0;
-        bool ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eper, k_eval_all, EVAL_T, 0) == cudaSuccess && eper >= 1;
+        bool ok = cudaFuncSetAttribute(k_eval_all, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EVAL_SMEM) == cudaSuccess &&
+                  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eper, k_eval_all, EVAL_T, EVAL_SMEM) == cudaSuccess && eper >= 1;
         bool seen_narrow = false;
         for (int i = (int)c->d - 1; i >= 0 && ok; i--) {
             const bool narrow = c->logs[i] <= EVAL_NARROW_LOG && c->logs[i + 1] <= EVAL_NARROW_LOG + 1;
@@ -347,7 +388,7 @@ int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outpu
     void *params[] = {&L, &d, &d_input, &d_outputs, &S, &cnt};
     cudaEvent_t ea = nullptr, eb = nullptr;
     if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
-    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_eval_all, dim3(fh->grid), dim3(EVAL_T), params, 0, st);
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_eval_all, dim3(fh->grid), dim3(EVAL_T), params, EVAL_SMEM, st);
     if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_EVAL, ea, eb); }
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
