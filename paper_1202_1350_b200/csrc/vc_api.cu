@@ -86,13 +86,14 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
         const vc_layer &L = layers[i];
         if (!L.type || !L.in1 || !L.in2) return VC_ERR_ARG;
         const uint64_t n = 1ull << L.log_size, nb = 1ull << c->logs[i + 1];
-        bool tree = true, onetype = true;
+        bool tree = true, self = true, onetype = true;
         for (uint64_t g = 0; g < n; g++) {
             if (L.type[g] > 3 || L.in1[g] >= nb || L.in2[g] >= nb) return VC_ERR_SHAPE;
             tree = tree && L.in1[g] == 2 * g && L.in2[g] == 2 * g + 1;
+            self = self && L.in1[g] == g && L.in2[g] == g;
             onetype = onetype && L.type[g] == L.type[0];
         }
-        c->wiring[i] = (tree ? 1u : 0u) | (onetype ? 2u : 0u);
+        c->wiring[i] = !onetype ? 0u : (tree ? 1u : (self ? 2u : 0u));
         c->h_type[i].assign(L.type, L.type + n);
         c->h_in1[i].assign(L.in1, L.in1 + n);
         c->h_in2[i].assign(L.in2, L.in2 + n);

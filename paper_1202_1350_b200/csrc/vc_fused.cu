@@ -115,13 +115,14 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
     for (; i >= 0; i--) {                         // grid-wide layers, separated by a counter rendezvous
         if (L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1) break;
         const uint32_t n = 1u << L[i].log_n;
-        const uint8_t *__restrict__ type = L[i].type;
-        const uint32_t *__restrict__ in1 = L[i].in1, *__restrict__ in2 = L[i].in2;
+        const Wires wr(L[i]);
         const uint64_t *Vb = L[i + 1].V;
         uint64_t *Vo = const_cast<uint64_t *>(L[i].V);
         eval_grid_barrier(cnt, gen);
         for (uint32_t g = b * EVAL_T + tid; g < n; g += G * EVAL_T) {
-            const uint64_t v = gate_f(type[g], __ldcg(Vb + in1[g]), __ldcg(Vb + in2[g]));
+            uint32_t i1, i2, t;
+            wr.get(g, i1, i2, t);
+            const uint64_t v = gate_f(t, __ldcg(Vb + i1), __ldcg(Vb + i2));
             Vo[g] = v;
             if (i == 0 && out0) out0[g] = v;
         }
@@ -143,7 +144,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
 #pragma unroll
         for (uint32_t k = 0; k < NG; k++) {
             const uint32_t g = k * EVAL_T + tid;
-            if (g < n) { rt[k] = __ldg(L[layer].type + g); ra[k] = __ldg(L[layer].in1 + g); rb[k] = __ldg(L[layer].in2 + g); }
+            if (g < n) Wires(L[layer]).get(g, ra[k], rb[k], rt[k]);
         }
     };
     fetch(i);
@@ -295,6 +296,8 @@ int fused_init(vc_circuit *c) {
         lp.in2 = i < c->d ? c->d_in2[i] : nullptr;
         lp.V = c->d_V[i];
         lp.log_n = c->logs[i];
+        lp.wiring = i < c->d ? c->wiring[i] : W_GENERIC;
+        lp.type0 = i < c->d ? c->h_type[i][0] : 0;
         if (i < c->d) {
             std::vector<CtaPlan> cta;
             plan_layer(c, i, fh.grid, lp, cta, smem_need);

@@ -48,11 +48,28 @@ struct LayerPlan {
     uint32_t thin;                       // != 0: at most one gate per worker thread: vc_fused_thin.cuh; the value = lanes per gate (1 or 4)
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
     uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
+    uint32_t wiring, type0;              // implicit wiring (W_TREE / W_SELF with the single gate type type0) or W_GENERIC
     uint32_t cap;                        // state capacity in gates (multiple of FT)
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
     uint32_t xw, yw;                     // words of the two fold buffers
     uint32_t off_tab, off_scr, off_commit;   // byte offsets in dynamic shared memory (after the state)
+};
+
+// Implicit wiring (§5.2: for regular circuits the in-neighbours of gate g are
+// computed from g instead of being read).  Layers with one gate type whose records are in1 = 2g, in2 = 2g+1 (the add
+// trees) or in1 = in2 = g (the squaring layers) are recognised at load; everything else reads its records.
+constexpr uint32_t W_GENERIC = 0, W_TREE = 1, W_SELF = 2;
+struct Wires {
+    const uint8_t *type;
+    const uint32_t *in1, *in2;
+    uint32_t mode, t0;
+    __device__ __forceinline__ explicit Wires(const LayerPlan &L) : type(L.type), in1(L.in1), in2(L.in2), mode(L.wiring), t0(L.type0) {}
+    __device__ __forceinline__ void get(uint32_t g, uint32_t &i1, uint32_t &i2, uint32_t &t) const {
+        if (mode == W_TREE) { i1 = 2 * g; i2 = 2 * g + 1; t = t0; }
+        else if (mode == W_SELF) { i1 = g; i2 = g; t = t0; }
+        else { i1 = __ldg(in1 + g); i2 = __ldg(in2 + g); t = __ldg(type + g); }
+    }
 };
 
 struct FusedArgs {

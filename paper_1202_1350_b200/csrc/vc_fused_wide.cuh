@@ -298,7 +298,9 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         if (res) { A.W = sW[l]; A.cP = sC[l]; A.idx = sI[l]; }
                         else {
                             A.W = a.P[g]; A.cP = a.C[g];
-                            A.idx = ph == 0 ? gin1[g] : (gin2[g] | ((gtype[g] == VC_RELAY ? 1u : 0u) << 31));
+                            uint32_t i1, i2, t;
+                            Wires(Lp).get(g, i1, i2, t);
+                            A.idx = ph == 0 ? i1 : (i2 | ((t == VC_RELAY ? 1u : 0u) << 31));
                         }
                         const uint32_t u = (A.idx & F_IDX_MASK) >> (j + 1);
                         ulonglong2 pr;
