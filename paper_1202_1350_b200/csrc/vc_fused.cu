@@ -1,5 +1,6 @@
 // vc_fused.cu — kernel + host driver (load-time plan, launch) of the on-chip schedule (see vc_fused.cuh).
 #include <algorithm>
+#include <cstdlib>
 #include <vector>
 
 #include "vc_circuit.hpp"
@@ -9,6 +10,11 @@
 
 namespace vc {
 
+// MASK: which layer kinds this instantiation contains (1 narrow single-CTA, 2 thin, 4 wide).  The whole proof can run in
+// the all-kinds kernel; when the layers of a circuit fall into few runs of {narrow, thin} and {wide}, each run is
+// launched in the kernel that holds only its own code (the proof state travels through DevState, as it does between
+// vc_prove_layer calls): the resident loop of the wide path then gets the registers of the kernel to itself.
+template <int MASK>
 __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
     extern __shared__ __align__(16) uint8_t smem[];
     FusedCtx &cx = *reinterpret_cast<FusedCtx *>(smem);
@@ -48,7 +54,7 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
         VC_TR(100 + layer);
         if (a.L[layer].kind == 0) {
-            if (blockIdx.x == 0) small_layer(a, cx, invfact, pas, dyn, layer, tr);
+            if (MASK & 1) { if (blockIdx.x == 0) small_layer(a, cx, invfact, pas, dyn, layer, tr); }
             handoff = true;
         } else {
             if (handoff) {
@@ -64,9 +70,12 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
                 __syncthreads();
                 handoff = false;
             }
-            if (a.L[layer].thin == 4) thin_layer<4>(a, cx, invfact, pas, dyn, layer, tr);
-            else if (a.L[layer].thin) thin_layer<1>(a, cx, invfact, pas, dyn, layer, tr);
-            else wide_layer(a, cx, invfact, pas, dyn, layer, tr);
+            if (a.L[layer].thin) {
+                if (MASK & 2) {
+                    if (a.L[layer].thin == 4) thin_layer<4>(a, cx, invfact, pas, dyn, layer, tr);
+                    else thin_layer<1>(a, cx, invfact, pas, dyn, layer, tr);
+                }
+            } else if (MASK & 4) wide_layer(a, cx, invfact, pas, dyn, layer, tr);
         }
         tr += 7 * (size_t)s + 1;
     }
@@ -170,6 +179,8 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
 constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
+constexpr size_t F_MAX_RUNS = 3;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
+static bool g_single_kernel = false;               // VC_SINGLE_KERNEL=1 in the environment at load: always the all-kinds kernel (A/B measurements)
 
 struct FusedHost {
     LayerPlan *d_plan = nullptr;
@@ -178,6 +189,7 @@ struct FusedHost {
     uint64_t *d_stamps = nullptr, *d_C = nullptr, *d_Tg = nullptr;
     unsigned long long *d_evcnt = nullptr;
     bool eval_ok = false;
+    std::vector<int> group;                        // per layer: 3 = narrow or thin, 4 = wide (which k_fused instantiation holds its code)
     int grid = 0;
     size_t smem = 0;
 };
@@ -305,12 +317,14 @@ int fused_init(vc_circuit *c) {
         }
     }
     fh.smem = smem_need;
-    if (cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess) {
+    if (cudaFuncSetAttribute(k_fused<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
+        cudaFuncSetAttribute(k_fused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
+        cudaFuncSetAttribute(k_fused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess) {
         (void)cudaGetLastError();
         return VC_OK;                                // no fused schedule on this device; streaming still works
     }
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fused, FT, fh.smem) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fused<7>, FT, fh.smem) != cudaSuccess || per_sm < 1) {
         (void)cudaGetLastError();
         return VC_OK;
     }
@@ -337,6 +351,9 @@ int fused_init(vc_circuit *c) {
         fh.eval_ok = ok;
     }
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
+    fh.group.resize(c->d);
+    for (uint32_t i = 0; i < c->d; i++) fh.group[i] = (h[i].kind == 0 || h[i].thin) ? 3 : 4;
+    if (const char *e = getenv("VC_SINGLE_KERNEL")) g_single_kernel = e[0] == '1';
     if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (!all_cta.empty() &&
@@ -362,16 +379,29 @@ int fused_supported(const vc_circuit *c, uint32_t) { return find(c) != nullptr; 
 int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {
     FusedHost *fh = find(c);
     if (!fh) return VC_ERR_STATE;
-    FusedArgs a;
-    a.L = fh->d_plan; a.d = c->d; a.begin = begin; a.end = end; a.seed = seed; a.st = c->d_state; a.tr = d_tr;
-    a.P = c->d_P; a.C = fh->d_C; a.T0 = c->d_T0; a.T1 = c->d_T1; a.Tg = fh->d_Tg; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
-    void *params[] = {&a};
-    cudaEvent_t ea = nullptr, eb = nullptr;
-    if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
-    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_fused, dim3(fh->grid), dim3(FT), params, fh->smem, st);
-    if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_FUSED_WIDE, ea, eb); }
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    // runs of layers by kernel group: {narrow, thin} -> k_fused<3>, {wide} -> k_fused<4>; more than F_MAX_RUNS runs -> one k_fused<7>
+    std::vector<std::pair<uint32_t, int>> runs;          // (first layer, mask)
+    for (uint32_t i = begin; i < end; i++) {
+        const int m = fh->group[i];
+        if (runs.empty() || runs.back().second != m) runs.emplace_back(i, m);
+    }
+    if (runs.size() > F_MAX_RUNS || g_single_kernel) { runs.clear(); runs.emplace_back(begin, 7); }
+    uint64_t off = 0;
+    for (size_t r = 0; r < runs.size(); r++) {
+        const uint32_t b0 = runs[r].first, e0 = r + 1 < runs.size() ? runs[r + 1].first : end;
+        FusedArgs a;
+        a.L = fh->d_plan; a.d = c->d; a.begin = b0; a.end = e0; a.seed = seed; a.st = c->d_state; a.tr = d_tr + off;
+        a.P = c->d_P; a.C = fh->d_C; a.T0 = c->d_T0; a.T1 = c->d_T1; a.Tg = fh->d_Tg; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
+        void *params[] = {&a};
+        const void *fn = runs[r].second == 3 ? (const void *)k_fused<3> : (runs[r].second == 4 ? (const void *)k_fused<4> : (const void *)k_fused<7>);
+        cudaEvent_t ea = nullptr, eb = nullptr;
+        if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
+        cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(fh->grid), dim3(FT), params, fh->smem, st);
+        if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_FUSED_WIDE, ea, eb); }
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+        for (uint32_t i = b0; i < e0; i++) off += 7ull * c->logs[i + 1] + 1;
+    }
     return VC_OK;
 }
 
