@@ -173,7 +173,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             const uint32_t l = k * FT + tid;
             const bool valid = l < ng;
             const uint32_t g = valid ? g0 + l : g0;
-            const uint32_t i1 = __ldg(gin1 + g), i2 = __ldg(gin2 + g), t = __ldg(gtype + g);
+            uint32_t i1, i2, t;
+            Wires(Lp).get(g, i1, i2, t);
             const uint64_t other = __ldg(Vb + i2);
             const uint64_t P = eb.eq_of(g);
             uint64_t W, c; uint32_t ign;
@@ -215,7 +216,8 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                     const uint32_t l = k * FT + tid;
                     const bool valid = l < ng;
                     const uint32_t g = valid ? g0 + l : g0;
-                    const uint32_t i1 = __ldg(gin1 + g), i2 = __ldg(gin2 + g), t = __ldg(gtype + g);
+                    uint32_t i1, i2, t;
+            Wires(Lp).get(g, i1, i2, t);
                     const uint64_t P = fp61::mul(e0.eq_of(g), e1.eq_of(i1));
                     uint64_t W, c; uint32_t ign;
                     gate_state(2, t, P, v1, W, c, ign);
