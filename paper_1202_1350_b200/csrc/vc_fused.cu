@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
 constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
-constexpr size_t F_MAX_RUNS = 3;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
+constexpr size_t F_MAX_RUNS = 4;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
 static bool g_single_kernel = false;               // VC_SINGLE_KERNEL=1 in the environment at load: always the all-kinds kernel (A/B measurements)
 
 struct FusedHost {
@@ -318,7 +318,8 @@ int fused_init(vc_circuit *c) {
     }
     fh.smem = smem_need;
     if (cudaFuncSetAttribute(k_fused<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
-        cudaFuncSetAttribute(k_fused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
+        cudaFuncSetAttribute(k_fused<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
+        cudaFuncSetAttribute(k_fused<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
         cudaFuncSetAttribute(k_fused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess) {
         (void)cudaGetLastError();
         return VC_OK;                                // no fused schedule on this device; streaming still works
@@ -352,7 +353,7 @@ int fused_init(vc_circuit *c) {
     }
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     fh.group.resize(c->d);
-    for (uint32_t i = 0; i < c->d; i++) fh.group[i] = (h[i].kind == 0 || h[i].thin) ? 3 : 4;
+    for (uint32_t i = 0; i < c->d; i++) fh.group[i] = h[i].kind == 0 ? 1 : (h[i].thin ? 2 : 4);
     if (const char *e = getenv("VC_SINGLE_KERNEL")) g_single_kernel = e[0] == '1';
     if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
@@ -393,7 +394,7 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         a.L = fh->d_plan; a.d = c->d; a.begin = b0; a.end = e0; a.seed = seed; a.st = c->d_state; a.tr = d_tr + off;
         a.P = c->d_P; a.C = fh->d_C; a.T0 = c->d_T0; a.T1 = c->d_T1; a.Tg = fh->d_Tg; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
         void *params[] = {&a};
-        const void *fn = runs[r].second == 3 ? (const void *)k_fused<3> : (runs[r].second == 4 ? (const void *)k_fused<4> : (const void *)k_fused<7>);
+        const void *fn = runs[r].second == 1 ? (const void *)k_fused<1> : runs[r].second == 2 ? (const void *)k_fused<2> : (runs[r].second == 4 ? (const void *)k_fused<4> : (const void *)k_fused<7>);
         cudaEvent_t ea = nullptr, eb = nullptr;
         if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
         cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(fh->grid), dim3(FT), params, fh->smem, st);

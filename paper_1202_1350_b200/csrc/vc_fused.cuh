@@ -70,6 +70,10 @@ struct Wires {
         else if (mode == W_SELF) { i1 = g; i2 = g; t = t0; }
         else { i1 = __ldg(in1 + g); i2 = __ldg(in2 + g); t = __ldg(type + g); }
     }
+    // one field at a time (the non-resident gate loop needs in1 alone in phase 1, in2 and the type in phase 2)
+    __device__ __forceinline__ uint32_t in1_of(uint32_t g) const { return mode == W_TREE ? 2 * g : (mode == W_SELF ? g : __ldg(in1 + g)); }
+    __device__ __forceinline__ uint32_t in2_of(uint32_t g) const { return mode == W_TREE ? 2 * g + 1 : (mode == W_SELF ? g : __ldg(in2 + g)); }
+    __device__ __forceinline__ uint32_t type_of(uint32_t g) const { return mode == W_GENERIC ? __ldg(type + g) : t0; }
 };
 
 struct FusedArgs {

@@ -145,8 +145,6 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     const uint32_t si = Lp.log_n, s = a.L[layer + 1].log_n;
     const bool res = Lp.resident != 0, has_ign = Lp.has_relay != 0;
     const uint64_t *__restrict__ Vb = a.L[layer + 1].V;
-    const uint8_t *__restrict__ gtype = Lp.type;
-    const uint32_t *__restrict__ gin1 = Lp.in1, *__restrict__ gin2 = Lp.in2;
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;
     const uint32_t nk = (ng + FT - 1) / FT;
@@ -168,13 +166,14 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     __syncthreads();
     uint64_t claim_part = 0;
     auto setup1 = [&](auto resident) {
+        const Wires wr(Lp);                      // records, or the rule that replaces them (built outside the loop: Lp sits in global memory)
 #pragma unroll 2
         for (uint32_t k = 0; k < nk; k++) {
             const uint32_t l = k * FT + tid;
             const bool valid = l < ng;
             const uint32_t g = valid ? g0 + l : g0;
             uint32_t i1, i2, t;
-            Wires(Lp).get(g, i1, i2, t);
+            wr.get(g, i1, i2, t);
             const uint64_t other = __ldg(Vb + i2);
             const uint64_t P = eb.eq_of(g);
             uint64_t W, c; uint32_t ign;
@@ -211,13 +210,14 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             const EqTab e1 = build_eq_tab(bufX + (2u << F_EQLOG), bufX + (3u << F_EQLOG), scr + 128, cx.r1, s, tid, FT);
             __syncthreads();
             auto setup2 = [&](auto resident) {
+                const Wires wr(Lp);
 #pragma unroll 2
                 for (uint32_t k = 0; k < nk; k++) {
                     const uint32_t l = k * FT + tid;
                     const bool valid = l < ng;
                     const uint32_t g = valid ? g0 + l : g0;
                     uint32_t i1, i2, t;
-            Wires(Lp).get(g, i1, i2, t);
+            wr.get(g, i1, i2, t);
                     const uint64_t P = fp61::mul(e0.eq_of(g), e1.eq_of(i1));
                     uint64_t W, c; uint32_t ign;
                     gate_state(2, t, P, v1, W, c, ign);
@@ -294,15 +294,15 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                     if (has_ign) hot_gates<true>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                     else hot_gates<false>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                 } else {
+                    const Wires wr(Lp);
                     for (uint32_t k = 0; k < nmine; k++) {
                         const uint32_t l = k * GT + tid, g = g0 + l;
                         GateIn A;
                         if (res) { A.W = sW[l]; A.cP = sC[l]; A.idx = sI[l]; }
                         else {
                             A.W = a.P[g]; A.cP = a.C[g];
-                            uint32_t i1, i2, t;
-                            Wires(Lp).get(g, i1, i2, t);
-                            A.idx = ph == 0 ? i1 : (i2 | ((t == VC_RELAY ? 1u : 0u) << 31));
+                            if (wr.mode == W_GENERIC) A.idx = ph == 0 ? wr.in1[g] : (wr.in2[g] | ((wr.type[g] == VC_RELAY ? 1u : 0u) << 31));
+                            else A.idx = ph == 0 ? wr.in1_of(g) : (wr.in2_of(g) | ((wr.t0 == VC_RELAY ? 1u : 0u) << 31));
                         }
                         const uint32_t u = (A.idx & F_IDX_MASK) >> (j + 1);
                         ulonglong2 pr;
