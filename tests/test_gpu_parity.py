@@ -130,6 +130,28 @@ def test_structured_small_circuits_bit_exact(vc, schedule):
         gc.close()
 
 
+def test_all_kinds_kernel_matches_the_split_launches(vc, monkeypatch):
+    """The proof runs either as one launch of the all-kinds kernel or as one launch per run of layer kinds (narrow / thin /
+    wide); VC_SINGLE_KERNEL=1 at load forces the former.  Both must give the oracle's transcript word for word: a circuit
+    whose kinds alternate (more runs than the split allows: all-kinds kernel by itself) and config 2 forced either way."""
+    c = W.random_circuit([3, 12, 5, 13, 2, 12, 6, 11], 9, 99)        # narrow / thin alternating: 8 runs
+    want_out, want_tr, _, _ = oracle.OracleCircuit(c).prove(c.input, 606)
+    for force in ("0", "1"):
+        monkeypatch.setenv("VC_SINGLE_KERNEL", force)
+        gc, out, tr = _gpu_prove(vc, c, 606)
+        assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), force
+        gc.close()
+    c2 = W.config(2)
+    g = _golden(2)
+    monkeypatch.setenv("VC_SINGLE_KERNEL", "1")
+    gc, out, tr = _gpu_prove(vc, c2, W.challenge_seed(2))
+    monkeypatch.setenv("VC_SINGLE_KERNEL", "0")
+    gc2, out2, tr2 = _gpu_prove(vc, c2, W.challenge_seed(2))
+    assert np.array_equal(tr, tr2) and np.array_equal(out, out2)
+    assert _sha(out) == g["outputs_sha256"]
+    gc.close(); gc2.close()
+
+
 # ------------------------------------------------------------------ full sizes: golden digests written by the oracle
 @pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
 def test_configs_match_oracle_golden(vc, k):
