@@ -148,7 +148,7 @@ def test_all_kinds_kernel_matches_the_split_launches(vc, monkeypatch):
     monkeypatch.setenv("VC_SINGLE_KERNEL", "0")
     gc2, out2, tr2 = _gpu_prove(vc, c2, W.challenge_seed(2))
     assert np.array_equal(tr, tr2) and np.array_equal(out, out2)
-    assert _sha(out) == g["outputs_sha256"]
+    assert _sha(out) == g["outputs_sha256"] and _sha(tr) == g["transcript_sha256"]
     gc.close(); gc2.close()
 
 
