@@ -275,7 +275,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         X = (X + 1) & ~(size_t)1; Y = (Y + 1) & ~(size_t)1;
         const size_t tabw = std::max<size_t>(X + Y, 4u << F_EQLOG);
         const size_t st_bytes = res ? state : 0;
-        const size_t commit_bytes = (size_t)F_WORKERS * 32;
+        const size_t commit_bytes = (size_t)FT * 32;
         const size_t total = std::max(F_FIXED_BYTES + st_bytes + tabw * 8 + scr_words * 8 + commit_bytes,
                                       F_FIXED_BYTES + fused_line_words(s, FT) * 8);   // the line restriction reuses the whole region
         if (total > F_SMEM_MAX) continue;

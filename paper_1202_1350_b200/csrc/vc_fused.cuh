@@ -300,6 +300,30 @@ __device__ __forceinline__ void round_rendezvous(const FusedArgs &a, uint32_t ep
 struct RoundPend { uint64_t *tr1, *tr2; uint32_t s1, s2; };
 // warp 15: the CTA totals t0..t2 (all lanes) go to the round's data words; CTA 0 converts the slot of two rounds ago
 // into transcript words and recycles the slot of epoch+2
+// the CTA totals t0..t2 (all lanes of the calling warp) are added to the round's six data words
+__device__ __forceinline__ void reducer_post_data(const FusedArgs &a, uint32_t ep, uint64_t t0, uint64_t t1, uint64_t t2) {
+    const uint32_t lane = threadIdx.x & 31;
+    unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
+    if (lane >= 1 && lane < 7) {
+        const uint32_t k = (lane - 1) >> 1;
+        const uint64_t v = k == 0 ? t0 : (k == 1 ? t1 : t2);
+        red_add(slot + lane, (((lane - 1) & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE);
+    }
+}
+// one warp per CTA: CTA 0 converts the slot of two rounds ago into transcript words, the last CTA recycles the slot of epoch+2
+__device__ __forceinline__ void reducer_housekeeping(const FusedArgs &a, uint32_t ep, uint64_t *tr, RoundPend &pd) {
+    const uint32_t lane = threadIdx.x & 31;
+    if (blockIdx.x == 0) {
+        if (pd.tr2) round_slot_to_transcript(a.slots + (size_t)pd.s2 * F_SLOT_WORDS, pd.tr2, lane);
+        pd.tr2 = pd.tr1; pd.s2 = pd.s1; pd.tr1 = tr; pd.s1 = ep % F_RING;
+    }
+    if (blockIdx.x == gridDim.x - 1) {
+        unsigned long long *z = a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS;
+#pragma unroll
+        for (int q = 0; q < F_SLOT_WORDS / 32; q++) z[q * 32 + lane] = 0ull;
+        __threadfence();
+    }
+}
 __device__ __forceinline__ void reducer_post(const FusedArgs &a, uint32_t ep, uint64_t t0, uint64_t t1, uint64_t t2, uint64_t *tr,
                                              RoundPend &pd) {
     const uint32_t lane = threadIdx.x & 31;

@@ -96,7 +96,7 @@ template <bool IGN>
 __device__ __forceinline__ void hot_gates(const bool UPD, uint64_t *sW, const uint64_t *sC, const uint32_t *sI,
                                           const uint64_t *tb, uint32_t j, uint32_t nmine, uint32_t tid, uint64_t r_prev,
                                           uint64_t omr, uint64_t (&s4)[4]) {
-    constexpr uint32_t GT = F_WORKERS;
+    constexpr uint32_t GT = FT;                  // all sixteen warps own gates on this path
     acc128 X0, X1, Y0, Y1; X0.clear(); X1.clear(); Y0.clear(); Y1.clear();
     const uint32_t sh = j + 1;
     auto one = [&](uint64_t &W, uint64_t cP, uint32_t idx, const ulonglong2 pr) {
@@ -148,8 +148,10 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     const CtaPlan cp = Lp.cta[b];
     const uint32_t g0 = cp.g0, ng = cp.g1 - cp.g0;
     const uint32_t nk = (ng + FT - 1) / FT;
-    constexpr uint32_t GT = F_WORKERS;           // warps 0..14 own the gates: l = k GT + tid; warp 15 is the reducer
-    const uint32_t nmine = (tid < GT && tid < ng) ? (ng - tid + GT - 1) / GT : 0;
+    constexpr uint32_t GT = FT;                  // all sixteen warps own gates: l = k GT + tid.  Between the commit barrier and the
+    // challenge warp 0 runs the rendezvous, warp 15 sums the committed words into the round's data words and warp 14 keeps
+    // the transcript (CTA 0) / recycles slots (last CTA): the three jobs share the rendezvous' latency
+    const uint32_t nmine = tid < ng ? (ng - tid + GT - 1) / GT : 0;
     ulonglong2 *cbuf = reinterpret_cast<ulonglong2 *>(dyn + Lp.off_commit);       // [GT][2]: X, X1, Y, Y1 sums per worker
     const uint32_t cap = Lp.cap;
     uint64_t *sW = reinterpret_cast<uint64_t *>(dyn);
@@ -244,21 +246,21 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         const uint32_t cnt = nbk << (K - j);
                         if (j == 1) {
                             const uint64_t *src = Vb + ((size_t)blo << K);
-                            if (tid < GT) fold_level_from_global(dst, src, cnt, r_prev, tid, GT);
+                            fold_level_from_global(dst, src, cnt, r_prev, tid, GT);
                         } else {
-                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
+                            for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
                         }
                         base = blo << (K - j);
                     } else {                     // the whole table: from the published level K-1 (j = K >= 2), from V (j = 1),
                         const uint32_t cnt = 1u << (s - j);                         // else from the previous buffer
                         if (j == 1 || j == K) {
                             const uint64_t *src = j == 1 ? Vb : a.Tg;
-                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) {
+                            for (uint32_t v = tid; v < cnt; v += GT) {
                                 const ulonglong2 p = __ldcg(reinterpret_cast<const ulonglong2 *>(src + 2 * (size_t)v));
                                 dst[v] = fold2(p.x, p.y, r_prev);
                             }
                         } else {
-                            if (tid < GT) for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
+                            for (uint32_t v = tid; v < cnt; v += GT) dst[v] = fold2(prev[2 * v], prev[2 * v + 1], r_prev);
                         }
                     }
                     tab = dst;
@@ -273,7 +275,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 if (j >= 1) {
                     uint64_t *Aout = (j & 1) ? a.T0 : a.T1;                          // level j
                     const uint32_t cnt = 1u << (s - j);
-                    if (tid < GT) for (uint32_t v = b * GT + tid; v < cnt; v += G * GT) {
+                    for (uint32_t v = b * GT + tid; v < cnt; v += G * GT) {
                         const ulonglong2 p = __ldcg(reinterpret_cast<const ulonglong2 *>(tab + 2 * (size_t)v));
                         __stcg(Aout + v, fold2(p.x, p.y, r_prev));
                     }
@@ -281,10 +283,10 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 fence = true;
             }
             VC_TR(13);
-            if (tid < GT) bar_workers();         // level j ready in shared memory (the reducer is still busy with round j-1)
+            __syncthreads();                     // level j ready in shared memory
             VC_TR(14);
             // ---- a4 (+ the pending a6 weight update): every gate of this CTA
-            if (tid < GT) {
+            {
                 const uint64_t omr = fp61::sub(1, r_prev);
                 const bool upd = j >= 1;
                 acc128 X, X1, Y, Y1; X.clear(); X1.clear(); Y.clear(); Y1.clear();
@@ -326,7 +328,6 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                     s4[0] = fp61::sub(fp61::add(s4[0], X.value()), s4[1]); s4[2] = fp61::sub(fp61::add(s4[2], Y.value()), s4[3]);
                 }
                 VC_TR(21);
-                if (!first) asm volatile("bar.sync 3, %0;" ::"r"((uint32_t)FT) : "memory");   // the reducer is done with round j-1's words
                 if (tid < ng) {                  // commit this worker's four canonical sums X0, X1, Y0, Y1
                     ulonglong2 o0, o1;
                     o0.x = s4[0]; o0.y = s4[1]; o1.x = s4[2]; o1.y = s4[3];
@@ -337,22 +338,23 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             __syncthreads();                     // every contribution of this CTA to message j is committed
             uint64_t *rslot = rr + j;
             if (warp == 15) {
-                // ---- a5, off the workers' critical path: sum the committed words, add them to the round's data words
+                // ---- a5 in the shadow of the rendezvous: sum the committed words, add them to the round's data words
                 const uint32_t nc = ng < GT ? ng : GT;
                 uint64_t Sl = 0, S1l = 0, Tl = 0, T1l = 0; uint32_t Sh = 0, S1h = 0, Th = 0, T1h = 0;
                 for (uint32_t i = lane; i < nc; i += 32) {
                     const ulonglong2 q0 = cbuf[2 * i], q1 = cbuf[2 * i + 1];
                     add_c(Sl, Sh, q0.x, 1u); add_c(S1l, S1h, q0.y, 1u); add_c(Tl, Th, q1.x, 1u); add_c(T1l, T1h, q1.y, 1u);
                 }
-                if (!(ph == 1 && j + 1 == s)) asm volatile("bar.arrive 3, %0;" ::"r"((uint32_t)FT) : "memory");   // words consumed
                 const uint64_t x = fp61::fold128(Sh, Sl), x1 = fp61::fold128(S1h, S1l), y = fp61::fold128(Th, Tl), y1 = fp61::fold128(T1h, T1l);
                 const uint64_t t0 = warp_sum61(x), t1 = warp_sum61(x1);
                 const uint64_t t2 = warp_sum61(fp61::sub(fp61::dbl(y1), y));        // x, y here are the bit-0 sums
-                reducer_post(a, ep, t0, t1, t2, tr, pd);
-            } else {
-                if (warp == 0) round_rendezvous(a, ep, fence, rslot, seed, ctr);   // ---- a6: rendezvous, then the challenge
-                bar_workers();
+                reducer_post_data(a, ep, t0, t1, t2);
+            } else if (warp == 14) {
+                reducer_housekeeping(a, ep, tr, pd);
+            } else if (warp == 0) {
+                round_rendezvous(a, ep, fence, rslot, seed, ctr);   // ---- a6: rendezvous, then the challenge
             }
+            __syncthreads();
             VC_TR(16);
             ctr++; tr += 3; ep++; first = false;
             r_prev = *rslot;                     // (the reducer does not use it)
@@ -372,7 +374,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
         }
     }
     if (tid == 0) { cx.ctr = ctr; cx.epoch = ep; }
-    if (warp == 15) reducer_flush(a, pd);                   // the last two rounds' messages
+    if (warp == 14) reducer_flush(a, pd);                   // the last two rounds' messages
     __syncthreads();
     VC_TR(17);
     // ---- a7: line restriction, all CTAs share the pass over V_{i+1}
