@@ -12,7 +12,8 @@
 //     the whole (<= 2^10-entry) table, redundantly; level K-1 is published through L2 once per phase;
 //   * a round ends in one grid rendezvous on a count word in L2 (atom.add + polling by one lane per CTA); warp 15 of
 //     every CTA (the "reducer") sums the CTA's committed contributions mod p and adds them to the round's six data
-//     words with red.add while the next round is already running; no kernel launch, no host round-trip.
+//     words with red.add — while the next round is already running on the thin path, in the shadow of the rendezvous on
+//     the wide path (where all sixteen warps own gates); no kernel launch, no host round-trip.
 // A challenge is only ever used AFTER every contribution to the message it answers has been committed (causality of
 // the interactive protocol), although the seeded generator would allow drawing it earlier; what is
 // pipelined is the summation of the committed contributions into the three transcript words.
@@ -262,7 +263,8 @@ __device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long lon
     return v;
 }
 
-// ---- warp-specialised rounds (vc_fused_thin.cuh, vc_fused_wide.cuh): warps 0..14 work, warp 15 reduces.
+// ---- warp-specialised rounds: vc_fused_thin.cuh has warps 0..14 work and warp 15 reduce beside them; vc_fused_wide.cuh
+// gives gates to all sixteen warps and splits the round's upkeep (rendezvous, reduction, transcript) over warps 0, 15, 14.
 constexpr uint32_t F_WORKERS = FT - 32;          // threads of warps 0..14
 __device__ __forceinline__ void bar_workers() { asm volatile("bar.sync 2, %0;" ::"r"(F_WORKERS) : "memory"); }
 // (hi:lo) += v if pred

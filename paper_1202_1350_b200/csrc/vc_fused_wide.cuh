@@ -357,7 +357,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             __syncthreads();
             VC_TR(16);
             ctr++; tr += 3; ep++; first = false;
-            r_prev = *rslot;                     // (the reducer does not use it)
+            r_prev = *rslot;
         }
         // ---- V~_{i+1}(r) = the two entries of level s-1 folded with the last challenge
         if (tid == 0) {
