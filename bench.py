@@ -207,6 +207,23 @@ def run_ours(args):
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
+    if args.layer_times:                         # per-layer device time of warm proofs (%globaltimer stamps of the fused kernels): not a bench value
+        best = None
+        for _ in range(5):
+            step()
+            torch.cuda.synchronize()
+            st = gc.layer_stamps().astype(np.int64)
+            dt = np.diff(st) / 1e3
+            best = dt if best is None else np.minimum(best, dt)
+        tot = 0.0
+        for i in range(c.d):
+            n, s = c.layers[i].log_size, c.log_below(i)
+            gr = (1 << n) * 2 * s
+            print(f"layer {i:3d} n=2^{n:2d} s={s:2d} rounds={2 * s:3d} {best[i]:9.1f} us {best[i] / (2 * s):8.2f} us/round {gr / best[i] / 1e3:9.2f} Ggr/s")
+            tot += best[i]
+        print(f"total us {tot:.3f} (min over 5 warm proofs, per layer; includes the launch gap where a new kernel starts)")
+        gc.close()
+        return
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.3)
@@ -254,11 +271,11 @@ def run_ours(args):
         L.vc_profile_enable(1)
         flush.fill_(1)
         step()
-        nk = 8
+        nk = 10
         pl, pm = (C.c_uint64 * nk)(), (C.c_double * nk)()
         L.vc_profile_read(pl, pm)
         L.vc_profile_enable(0)
-        kinds = ["evaluate", "setup(beta,start)", "round", "update+fold", "line", "fused_small", "fused_wide", "misc"]
+        kinds = ["evaluate", "setup(beta,start)", "round", "update+fold", "line", "fused_narrow", "fused_wide", "misc", "fused_thin", "cluster"]
         prof = {kinds[i]: {"launches": int(pl[i]), "ms": round(float(pm[i]), 4)} for i in range(nk) if pl[i]}
         prof_total = sum(v["ms"] for v in prof.values())
         dom = max(prof, key=lambda n: prof[n]["ms"])
@@ -358,6 +375,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")
     ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
     args = ap.parse_args()

@@ -136,8 +136,8 @@ int vc_bench_modmul(uint32_t grid, uint32_t block, uint32_t iters, uint32_t ilp,
 /* Per-kernel-kind device timing (bench.py's roofline): when enabled, every launch is bracketed by CUDA events on
  * its stream; vc_profile_read synchronises the device, sums launches and milliseconds per kind into two arrays of
  * VC_K_COUNT entries, and clears the records.  Enabling costs host time per launch: never on during a timed step. */
-enum { VC_K_EVAL = 0, VC_K_SETUP = 1, VC_K_ROUND = 2, VC_K_UPDATE = 3, VC_K_LINE = 4, VC_K_FUSED_SMALL = 5,
-       VC_K_FUSED_WIDE = 6, VC_K_MISC = 7, VC_K_COUNT = 8 };
+enum { VC_K_EVAL = 0, VC_K_SETUP = 1, VC_K_ROUND = 2, VC_K_UPDATE = 3, VC_K_LINE = 4, VC_K_FUSED_NARROW = 5,
+       VC_K_FUSED_WIDE = 6, VC_K_MISC = 7, VC_K_FUSED_THIN = 8, VC_K_CLUSTER = 9, VC_K_COUNT = 10 };
 int vc_profile_enable(int on);
 int vc_profile_read(uint64_t *launches, double *ms);
 

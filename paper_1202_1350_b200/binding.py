@@ -237,6 +237,12 @@ class Circuit:
         _check(lib().vc_debug_state(self.handle, z.ctypes.data, C.byref(claim), C.byref(ctr), _stream_ptr(None)), "vc_debug_state")
         return z, int(claim.value), int(ctr.value)
 
+    def layer_stamps(self) -> np.ndarray:
+        """d+1 device timestamps (ns) of the last fused proof: start of each layer, [d] = end (vc_debug_layer_stamps)."""
+        h = np.zeros(self.d + 1, dtype=np.uint64)
+        _check(lib().vc_debug_layer_stamps(self.handle, _host_ptr(h), None), "vc_debug_layer_stamps")
+        return h
+
     def flags(self) -> int:
         f = C.c_uint32(0)
         _check(lib().vc_status(self.handle, C.byref(f), _stream_ptr(None)), "vc_status")

@@ -29,7 +29,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and SO.exists() and SO.stat().st_mtime >= newest_source_mtime():
         return SO
     tmp = SO.with_suffix(f".tmp{os.getpid()}.so")
-    cmd = [nvcc()] + NVCC_FLAGS + ["-o", str(tmp)] + [str(CSRC / s) for s in SOURCES]
+    extra = os.environ.get("VC_NVCC_EXTRA", "").split()      # e.g. -DVC_TRACE / -DVC_POISON debug builds
+    cmd = [nvcc()] + NVCC_FLAGS + extra + ["-o", str(tmp)] + [str(CSRC / s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(" ".join(cmd))

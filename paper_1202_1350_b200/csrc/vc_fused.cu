@@ -4,6 +4,7 @@
 #include <vector>
 
 #include "vc_circuit.hpp"
+#include "vc_cluster.cuh"
 #include "vc_fused_small.cuh"
 #include "vc_fused_thin.cuh"
 #include "vc_fused_wide.cuh"
@@ -179,7 +180,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
 constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
-constexpr size_t F_MAX_RUNS = 4;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
+constexpr size_t F_MAX_RUNS = 8;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
 static bool g_single_kernel = false;               // VC_SINGLE_KERNEL=1 in the environment at load: always the all-kinds kernel (A/B measurements)
 
 struct FusedHost {
@@ -189,9 +190,12 @@ struct FusedHost {
     uint64_t *d_stamps = nullptr, *d_C = nullptr, *d_Tg = nullptr;
     unsigned long long *d_evcnt = nullptr;
     bool eval_ok = false;
-    std::vector<int> group;                        // per layer: 3 = narrow or thin, 4 = wide (which k_fused instantiation holds its code)
+    std::vector<int> group;                        // per layer: 1 narrow, 2 thin, 4 wide (which k_fused instantiation holds its code), 8 = the cluster engine
     int grid = 0;
     size_t smem = 0;
+    ClLayer *d_cl = nullptr;                       // the cluster engine's plans (vc_cluster.cuh)
+    int csize = 0;                                 // CTAs per cluster (0: engine unavailable)
+    size_t cl_smem = 0;
 };
 static std::vector<std::pair<const vc_circuit *, FusedHost>> g_fused;
 
@@ -292,6 +296,88 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
     // unreachable: the last attempt (non-resident, no slices) needs only the fixed buffers
 }
 
+// ---- the cluster engine's load-time plan (vc_cluster.cuh): how many CTAs take a layer, which block of V_{i+1} each
+// CTA's gates read in each phase, how the line restriction is blocked.  Index bookkeeping on the host copy of the records.
+static size_t cl_line_words(uint32_t s, uint32_t tb) {
+    const size_t sp = s < 3 ? 3 : s, P = tb + 4, NB = (size_t)1 << tb;
+    return (((s + 1) * sp + 1) & ~(size_t)1) + NB * P + (NB * P + 1) / 2 + 1 + 64 + 8;
+}
+static bool plan_cluster_layer(const vc_circuit *c, uint32_t i, int csize, ClLayer &cl, size_t &dyn_bytes) {
+    static const int target_gpc = getenv("VC_CL_GPC") ? atoi(getenv("VC_CL_GPC")) : 256;
+    static const int single_max = getenv("VC_CL_SINGLE") ? atoi(getenv("VC_CL_SINGLE")) : 512;
+    const uint32_t si = c->logs[i], s = c->logs[i + 1];
+    cl = ClLayer{};
+    if (si > CL_MAX_N || s > CL_MAX_S) return false;
+    const uint32_t n = 1u << si;
+    uint32_t A = 1;
+    if ((int)n > single_max) { while (A < (uint32_t)csize && n / A > (uint32_t)target_gpc) A <<= 1; }
+    while (n / A > (uint32_t)CL_GT) { if (A >= (uint32_t)csize) return false; A <<= 1; }
+    if (A > n) A = n;
+    const uint32_t gpc = n / A;
+    uint32_t mmax = 1;
+    for (int ph = 0; ph < 2; ph++) {
+        const std::vector<uint32_t> &idx = ph == 0 ? c->h_in1[i] : c->h_in2[i];
+        uint32_t m = 1, blk[CL_C] = {0};
+        for (uint32_t b = 0; b < A; b++) {
+            uint32_t lo = 0xffffffffu, hi = 0;
+            for (uint32_t g = b * gpc; g < (b + 1) * gpc; g++) { lo = std::min(lo, idx[g]); hi = std::max(hi, idx[g]); }
+            while ((lo >> m) != (hi >> m)) m++;
+            blk[b] = lo;
+        }
+        bool sliced = A > 1 && m < s && (1u << (s - m)) == A;
+        if (sliced) {                            // the A blocks must be the A distinct aligned blocks of the table
+            uint32_t seen = 0;
+            for (uint32_t b = 0; b < A; b++) seen |= 1u << (blk[b] >> m);
+            sliced = seen == (A == 32 ? 0xffffffffu : (1u << A) - 1);
+        }
+        if (!sliced) m = s;
+        if (m > CL_MAX_M) return false;
+        cl.m[ph] = m;
+        for (uint32_t b = 0; b < A; b++) cl.blk[ph][b] = sliced ? blk[b] >> m : 0;
+        mmax = std::max(mmax, m);
+    }
+    cl.A = A; cl.gpc = gpc;
+    uint32_t nact = std::max<uint32_t>(gpc, std::min<uint32_t>(CL_GT, 1u << (mmax - 1)));
+    if (si > 6) nact = std::max<uint32_t>(nact, 192);
+    cl.nact = std::min<uint32_t>(CL_GT, (nact + 31) & ~31u);
+    uint32_t la = 0; while ((1u << la) < A) la++;
+    if (s < la) return false;
+    cl.sb = s - la;
+    const size_t tabw = std::max<size_t>((size_t)1 << mmax, 64) + std::max<size_t>((size_t)1 << (mmax - 1), 64);
+    cl.off_line = (uint32_t)(tabw * 8);
+    size_t need = tabw * 8;
+    cl.ltb = 0; cl.lthr = 32;
+    if (s == 1) cl.lmode = CL_LINE_NONE;
+    else if (cl.sb < 3) cl.lmode = CL_LINE_DIRECT;
+    else {
+        const size_t nE = (size_t)1 << (cl.sb - 3), lw = nE * (s - 1) + std::max<size_t>(nE / 2, 1) * (s - 1) + 2;
+        if (lw * 8 <= 72 * 1024) { cl.lmode = CL_LINE_STREAM; need += lw * 8; }
+        else {
+            // a separate pass after the rounds: blocks of 2^tb threads x 8 words, at least one block per active CTA when the table allows it
+            cl.lmode = CL_LINE_PASS;
+            const uint32_t sp = s < 3 ? 3 : s;
+            uint32_t tb = fused_line_tb(s, CL_GT);
+            const uint32_t cap = sp - 3 > la ? sp - 3 - la : 0;
+            tb = std::min(tb, cap);
+            cl.ltb = tb;
+            cl.lthr = std::max<uint32_t>(32, 1u << tb);
+            need = std::max(need, cl_line_words(s, tb) * 8);
+        }
+    }
+    dyn_bytes = std::max(dyn_bytes, need);
+    return true;
+}
+
+static cudaError_t launch_cluster(const ClArgs &a, int csize, size_t smem, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(csize); cfg.blockDim = dim3(CL_T); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_cluster, a);
+}
+
 int fused_init(vc_circuit *c) {
     if (!c->coop_ok) return VC_OK;
     FusedHost fh;
@@ -355,6 +441,42 @@ int fused_init(vc_circuit *c) {
     fh.group.resize(c->d);
     for (uint32_t i = 0; i < c->d; i++) fh.group[i] = h[i].kind == 0 ? 1 : (h[i].thin ? 2 : 4);
     if (const char *e = getenv("VC_SINGLE_KERNEL")) g_single_kernel = e[0] == '1';
+    {   // the cluster engine takes every layer it can plan (VC_NO_CLUSTER=1: never, for A/B measurements)
+        const char *nc = getenv("VC_NO_CLUSTER");
+        std::vector<ClLayer> hc(c->d);
+        size_t dyn = 0;
+        const size_t fixed = (sizeof(ClShared) + 15) & ~(size_t)15;
+        int csize = 0;
+        if (!(nc && nc[0] == '1') && !g_single_kernel &&
+            cudaFuncSetAttribute(k_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
+            cudaFuncSetAttribute(k_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) == cudaSuccess) {
+            for (int cs : {CL_C, CL_C / 2}) {
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3(cs); cfg.blockDim = dim3(CL_T); cfg.dynamicSmemBytes = F_SMEM_MAX;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeClusterDimension;
+                at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                int ncl = 0;
+                if (cudaOccupancyMaxActiveClusters(&ncl, k_cluster, &cfg) == cudaSuccess && ncl >= 1) { csize = cs; break; }
+                (void)cudaGetLastError();
+            }
+        }
+        (void)cudaGetLastError();
+        bool any = false;
+        if (csize) {
+            for (uint32_t i = 0; i < c->d; i++) {
+                size_t need = dyn;
+                if (plan_cluster_layer(c, i, csize, hc[i], need) && fixed + need <= F_SMEM_MAX) { dyn = need; fh.group[i] = 8; any = true; }
+                else hc[i] = ClLayer{};
+            }
+        }
+        if (any) {
+            if (cudaMalloc(&fh.d_cl, hc.size() * sizeof(ClLayer)) != cudaSuccess) return VC_ERR_NOMEM;
+            if (cudaMemcpy(fh.d_cl, hc.data(), hc.size() * sizeof(ClLayer), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
+            fh.csize = csize; fh.cl_smem = fixed + dyn;
+        }
+    }
     if (cudaMemset(fh.d_stamps, 0, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemcpy(fh.d_plan, h.data(), h.size() * sizeof(LayerPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (!all_cta.empty() &&
@@ -368,7 +490,7 @@ void fused_free(const vc_circuit *c) {
     for (size_t i = 0; i < g_fused.size(); i++)
         if (g_fused[i].first == c) {
             FusedHost &f = g_fused[i].second;
-            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg); cudaFree(f.d_evcnt);
+            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg); cudaFree(f.d_evcnt); cudaFree(f.d_cl);
             g_fused.erase(g_fused.begin() + i);
             return;
         }
@@ -386,7 +508,12 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         const int m = fh->group[i];
         if (runs.empty() || runs.back().second != m) runs.emplace_back(i, m);
     }
-    if (runs.size() > F_MAX_RUNS || g_single_kernel) { runs.clear(); runs.emplace_back(begin, 7); }
+    if (runs.size() > F_MAX_RUNS || g_single_kernel) {   // the all-kinds kernel cannot hold cluster layers: they keep their own launches
+        bool has_cl = false;
+        for (auto &r : runs) has_cl = has_cl || r.second == 8;
+        if (!has_cl) { runs.clear(); runs.emplace_back(begin, 7); }
+        else for (auto &r : runs) if (r.second != 8) r.second = 7;
+    }
     uint64_t off = 0;
     for (size_t r = 0; r < runs.size(); r++) {
         const uint32_t b0 = runs[r].first, e0 = r + 1 < runs.size() ? runs[r + 1].first : end;
@@ -394,11 +521,23 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         a.L = fh->d_plan; a.d = c->d; a.begin = b0; a.end = e0; a.seed = seed; a.st = c->d_state; a.tr = d_tr + off;
         a.P = c->d_P; a.C = fh->d_C; a.T0 = c->d_T0; a.T1 = c->d_T1; a.Tg = fh->d_Tg; a.slots = fh->d_slots; a.stamps = fh->d_stamps;
         void *params[] = {&a};
-        const void *fn = runs[r].second == 1 ? (const void *)k_fused<1> : runs[r].second == 2 ? (const void *)k_fused<2> : (runs[r].second == 4 ? (const void *)k_fused<4> : (const void *)k_fused<7>);
+        const int mask = runs[r].second;
+        const void *fn = mask == 1 ? (const void *)k_fused<1> : mask == 2 ? (const void *)k_fused<2> : (mask == 4 ? (const void *)k_fused<4> : (const void *)k_fused<7>);
         cudaEvent_t ea = nullptr, eb = nullptr;
         if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
-        cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(fh->grid), dim3(FT), params, fh->smem, st);
-        if (g_profile) { cudaEventRecord(eb, st); prof_push(VC_K_FUSED_WIDE, ea, eb); }
+        cudaError_t e;
+        if (mask == 8) {
+            ClArgs ca;
+            ca.L = fh->d_plan; ca.cl = fh->d_cl; ca.d = c->d; ca.begin = b0; ca.end = e0; ca.csize = (uint32_t)fh->csize; ca.seed = seed;
+            ca.st = c->d_state; ca.tr = d_tr + off; ca.stamps = fh->d_stamps;
+            e = launch_cluster(ca, fh->csize, fh->cl_smem, st);
+        } else {
+            e = cudaLaunchCooperativeKernel(fn, dim3(fh->grid), dim3(FT), params, fh->smem, st);
+        }
+        if (g_profile) {
+            cudaEventRecord(eb, st);
+            prof_push(mask == 8 ? VC_K_CLUSTER : mask == 1 ? VC_K_FUSED_NARROW : mask == 2 ? VC_K_FUSED_THIN : VC_K_FUSED_WIDE, ea, eb);
+        }
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
         for (uint32_t i = b0; i < e0; i++) off += 7ull * c->logs[i + 1] + 1;
