@@ -32,19 +32,21 @@
 
 namespace vc {
 
-constexpr int CL_GT = 512;                  // gate / fold threads per CTA (warps 0..15)
-constexpr int CL_LT = 96;                   // line threads (warps 16..18)
-constexpr int CL_T = CL_GT + CL_LT + 32;    // + the service warp (warp 19): 640 threads keep 96 registers each
+constexpr int CL_GW = 256;                  // gate threads per CTA (warps 0..7): one gate each
+constexpr int CL_FW = 256;                  // fold threads (warps 8..15): the fold tables and the challenges
+constexpr int CL_GT = CL_GW + CL_FW;
+constexpr int CL_LT = 64;                   // line threads (warps 16, 17)
+constexpr int CL_T = CL_GT + CL_LT + 64;    // + the transcript warp (18) and the service warp (19): 640 threads keep 96 registers each
 constexpr int CL_C = 16;                    // CTAs per cluster
 constexpr uint32_t CL_MAX_M = 13;           // a CTA's level-0 slice: at most 2^13 entries
 constexpr uint32_t CL_MAX_S = 14;           // table below: at most 2^14 entries
-constexpr uint32_t CL_MAX_N = 13;           // gates: at most 2^13 (16 CTAs x 512)
+constexpr uint32_t CL_MAX_N = 12;           // gates: at most 2^12 (16 CTAs x 256)
 constexpr uint32_t CL_LINE_NONE = 0, CL_LINE_STREAM = 1, CL_LINE_DIRECT = 2, CL_LINE_PASS = 3;
 
 struct ClLayer {                            // load-time plan of one layer (A = 0: not run by this engine)
     uint32_t A;                             // active CTAs (power of two)
     uint32_t gpc;                           // gates per active CTA
-    uint32_t nact;                          // threads per CTA that take part in the rounds (multiple of 32)
+    uint32_t ngt, nft;                      // gate threads (tid < ngt) and fold threads (256 <= tid < 256 + nft) that take part, multiples of 32
     uint32_t m[2];                          // per phase: log2 entries of a CTA's level-0 slice (== s: the whole table)
     uint32_t blk[2][CL_C];                  // per phase and CTA: its slice is entries [blk << m, (blk + 1) << m)
     uint32_t lmode;                         // how q[2..s] are computed: CL_LINE_*
@@ -64,6 +66,9 @@ struct ClArgs {
     uint64_t *stamps;                       // d+1 words: %globaltimer when CTA 0 starts layer i
 };
 
+constexpr uint32_t CL_MAX_LAYERS = 24;      // layers per launch (their plans are copied to shared memory; longer runs are split by the host)
+struct ClPlanS { ClLayer C; LayerPlan Lp; const uint64_t *Vb; uint32_t s, pad; };   // one layer's plan, the table below it and its log size
+
 struct ClShared {
     FusedCtx cx;
     uint64_t invfact[MAX_VARS + 1];
@@ -76,6 +81,8 @@ struct ClShared {
     uint64_t mb_state;                      // (z, claim, ctr) from CTA 0 for a CTA that joins a wider layer
     volatile uint32_t rounds_done;          // rounds of the current layer handed off so far (read by the line and service warps)
     volatile uint32_t svc_done;             // rounds of the current layer whose commit buffer the service warp has summed
+    volatile uint32_t tr_done;              // CTA 0: rounds of the current layer the transcript warp has written
+    uint32_t pad1;
     alignas(16) uint64_t inbox[8][CL_C][4]; // CTA 0: per round (mod 8: the service warps of the other CTAs run up to five rounds ahead of CTA 0's) and CTA: G0, G1, G2, start-claim share
     alignas(16) uint64_t qin[2][CL_C][16];  // per layer parity and CTA: q[2..s] shares
     alignas(16) uint64_t gat[2][64];        // per phase: level m-1 of the fold table, all blocks
@@ -83,7 +90,10 @@ struct ClShared {
     uint64_t eqlo[128], eqhi[128];          // beta(z, g) = eqlo[g & 127] eqhi[g >> 7]
     uint64_t dk[32];                        // Lagrange denominators of the nodes 0..s: (-1)^(s-k) / (k! (s-k)!)
     uint64_t lpts[32];                      // line warps: l(t)_k of the level being folded, t = 2..s
-    alignas(16) ulonglong2 cbuf[4][CL_GT];  // committed products: a ring of four rounds (the service warp runs behind the gates)
+    alignas(16) ClPlanS pl[CL_MAX_LAYERS];  // the plans of layers begin .. end-1
+    alignas(16) ulonglong2 cbuf[4][CL_GW];  // committed products: a ring of four rounds (the service warp runs behind the gates)
+    alignas(16) uint64_t chal[2][2];        // (r, 1 - r) of round jj in slot jj & 1: written by the dealer before the round's commit barrier,
+                                            // read by everyone after the hand-off
 #ifdef VC_TRACE
     uint32_t trc[768][8];                   // CTA 0 / thread 0: SM clock at marked points, one row per round or layer
     uint32_t trn;
@@ -141,196 +151,226 @@ __device__ __forceinline__ uint64_t cl_mul_lazy(uint64_t W, uint64_t m) {
     const uint64_t lo = W * m, hi = fp61::mulhi(W, m);
     return (lo & fp61::P) + ((lo >> 61) | (hi << 3));
 }
-// service warp: the CTA's three sums of one message from its commit buffer (x | bit << 63, y), every lane gets all three.
-// Per lane four 96-bit sums (all x, x with bit 1, all y, y with bit 1); across the lanes REDUX on 27/27/19-bit pieces.
-__device__ __forceinline__ uint64_t cl_warp_sum96(uint64_t lo, uint32_t hi) {       // hi < 2^9 (at most 16 words per lane)
-    uint32_t p0 = (uint32_t)lo & 0x7ffffffu, p1 = (uint32_t)(lo >> 27) & 0x7ffffffu, p2 = (uint32_t)(lo >> 54) | (hi << 10);
-    p0 = __reduce_add_sync(0xffffffffu, p0);
-    p1 = __reduce_add_sync(0xffffffffu, p1);
-    p2 = __reduce_add_sync(0xffffffffu, p2);          // < 2^24: counts units of 2^54
-    // 2^54 * p2 = 2^54 (p2 & 127) + 2^61 (p2 >> 7) = 2^54 (p2 & 127) + (p2 >> 7)  (mod p)
-    const uint64_t x = (uint64_t)p0 + ((uint64_t)p1 << 27) + ((uint64_t)(p2 & 127u) << 54) + (p2 >> 7);
-    return fp61::reduce62(x);                          // x < 2^32 + 2^59 + 2^61 + 2^17
-}
-__device__ __noinline__ void cl_svc_sums(const ulonglong2 *cb, uint32_t gpc, uint64_t &t0, uint64_t &t1, uint64_t &t2) {
+// service warp: the CTA's three sums of one message from its commit buffer (x | bit << 63, y').  Per lane three 96-bit
+// sums (all x, x with bit 1, all y'); across the lanes REDUX on 27/27/19-bit pieces; lane k < 3 then assembles value k:
+// lane 0: G0 = sum x - sum_{bit 1} x, lane 1: G1 = sum_{bit 1} x, lane 2: G2 = sum y'.  Returns this lane's value.
+__device__ __noinline__ uint64_t cl_svc_sums(const ulonglong2 *cb, uint32_t gpc) {
     const uint32_t lane = threadIdx.x & 31;
-    uint64_t Sl = 0, S1l = 0, Tl = 0, T1l = 0; uint32_t Sh = 0, S1h = 0, Th = 0, T1h = 0;
+    uint64_t Sl = 0, S1l = 0, Tl = 0; uint32_t Sh = 0, S1h = 0, Th = 0;
 #pragma unroll 1
     for (uint32_t i = lane; i < gpc; i += 32) {
-        const ulonglong2 q = cb[i];
+        const ulonglong2 q = cb[i];                          // (W (x_b + c) | bit << 63,  chi(bit, 2) W (x_2 + c)), both unreduced
         const uint32_t bit = (uint32_t)(q.x >> 63);
         const uint64_t v1 = q.x & ~(1ull << 63);
-        add_c(Sl, Sh, v1, 1u); add_c(S1l, S1h, v1, bit);
-        add_c(Tl, Th, q.y, 1u); add_c(T1l, T1h, q.y, bit);
+        add_c(Sl, Sh, v1, 1u); add_c(S1l, S1h, v1, bit); add_c(Tl, Th, q.y, 1u);
     }
-    const uint64_t x = cl_warp_sum96(Sl, Sh), x1 = cl_warp_sum96(S1l, S1h), y = cl_warp_sum96(Tl, Th), y1 = cl_warp_sum96(T1l, T1h);
-    t0 = fp61::sub(x, x1);
-    t1 = x1;
-    t2 = fp61::sub(fp61::add(fp61::dbl(y1), y1), y);
+    uint32_t pc[9];                                          // hi < 2^4 (at most 8 words per lane): top piece < 2^14, its sum < 2^19
+    pc[0] = (uint32_t)Sl & 0x7ffffffu;  pc[1] = (uint32_t)(Sl >> 27) & 0x7ffffffu;  pc[2] = (uint32_t)(Sl >> 54) | (Sh << 10);
+    pc[3] = (uint32_t)S1l & 0x7ffffffu; pc[4] = (uint32_t)(S1l >> 27) & 0x7ffffffu; pc[5] = (uint32_t)(S1l >> 54) | (S1h << 10);
+    pc[6] = (uint32_t)Tl & 0x7ffffffu;  pc[7] = (uint32_t)(Tl >> 27) & 0x7ffffffu;  pc[8] = (uint32_t)(Tl >> 54) | (Th << 10);
+#pragma unroll
+    for (int k = 0; k < 9; k++) pc[k] = __reduce_add_sync(0xffffffffu, pc[k]);
+    const uint32_t q = lane == 2 ? 2u : 1u;                  // lanes 0 and 1 assemble sum_{bit 1} x, lane 2 sum y'; lane 0 also sum x
+    const uint32_t a0 = q == 2 ? pc[6] : pc[3], a1 = q == 2 ? pc[7] : pc[4], a2 = q == 2 ? pc[8] : pc[5];
+    // 2^54 * a2 = 2^54 (a2 & 127) + 2^61 (a2 >> 7) = 2^54 (a2 & 127) + (a2 >> 7)  (mod p)
+    uint64_t v = fp61::reduce62((uint64_t)a0 + ((uint64_t)a1 << 27) + ((uint64_t)(a2 & 127u) << 54) + (a2 >> 7));
+    if (lane == 0) {
+        const uint64_t x = fp61::reduce62((uint64_t)pc[0] + ((uint64_t)pc[1] << 27) + ((uint64_t)(pc[2] & 127u) << 54) + (pc[2] >> 7));
+        v = fp61::sub(x, v);
+    }
+    return v;
 }
 
 struct ClPhases { uint32_t rd[2], gat[2], dat[8], end[2], state; };   // parity of the next phase to wait for, per mbarrier
 
-// The rounds of one layer in an active CTA: gate / fold threads (tid < nact) and the service warp.
-__device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t *dyn, uint32_t layer, uint64_t *tr, uint32_t rank,
-                                          ClPhases &php) {
+// Round numbering.  R counts the rounds this CTA has taken part in since the launch (it indexes the commit ring and the
+// counters rounds_done / svc_done); Q counts the rounds of layers run by more than one CTA (the same in every CTA: it
+// indexes CTA 0's inbox ring and tr_done).
+// ---- the service warp (a5, behind the gates): this CTA's sums of every message go to CTA 0's inbox (A > 1) or straight to
+// the transcript (A = 1).  It follows the hand-offs through rounds_done and frees the commit buffers through svc_done;
+// it runs through all layers of the launch on its own, a few messages behind the gates, and is on nobody's critical path.
+__device__ __forceinline__ void cl_svc_role(const ClArgs &a, ClShared &S, uint32_t rank) {
+    const uint32_t lane = threadIdx.x & 31;
+    uint64_t *tr = a.tr;
+    uint32_t R = 0, Q = 0;
+    for (uint32_t layer = a.begin; layer < a.end; layer++) {
+        const ClLayer &C = S.pl[layer - a.begin].C;
+        const uint32_t s = S.pl[layer - a.begin].s, A = C.A, gpc = C.gpc, ngw = (gpc + 31) >> 5;
+        if (rank < A) {
+#pragma unroll 1
+            for (uint32_t jj = 0; jj < 2 * s; jj++, R++) {
+                while (S.rounds_done < R + 1) { }
+                if (rank == 0 && A > 1) while (S.tr_done + 4 < Q + jj + 1) { }   // bounds how far the inbox writers run ahead
+                uint64_t mine = cl_svc_sums(S.cbuf[R & 3], gpc);
+                __syncwarp();
+                if (lane == 0) S.svc_done = R + 1;
+                if (layer == 0 && jj == 0) {                 // a2: the start claim's share rides with message 0
+                    const uint64_t t3 = warp_sum61(lane < ngw ? S.cx.red[lane] : 0);
+                    if (lane == 3) mine = t3;
+                }
+                if (A == 1) {                                // the CTA's sums are the message
+                    if (lane < 3) tr[3 * jj + lane] = mine;
+                    if (layer == 0 && jj == 0 && lane == 3) a.st->G[3] = mine;
+                } else if (lane < 4) {
+                    const uint32_t k = (Q + jj) & 7;
+                    cl_st_async(cl_mapa(cl_smem(&S.inbox[k][rank][lane]), 0), mine, cl_mapa(cl_smem(&S.mb_dat[k]), 0));
+                }
+            }
+        }
+        if (A > 1) Q += 2 * s;
+        tr += 7 * (size_t)s + 1;
+    }
+}
+// ---- the transcript warp of CTA 0: message jj of a layer run by A > 1 CTAs = the sum of the A shares in its inbox slot
+__device__ __forceinline__ void cl_tr_role(const ClArgs &a, ClShared &S) {
+    const uint32_t lane = threadIdx.x & 31;
+    uint64_t *tr = a.tr;
+    uint32_t Q = 0, phase[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (uint32_t layer = a.begin; layer < a.end; layer++) {
+        const uint32_t s = S.pl[layer - a.begin].s, A = S.pl[layer - a.begin].C.A;
+        if (A > 1) {
+#pragma unroll 1
+            for (uint32_t jj = 0; jj < 2 * s; jj++, Q++) {
+                const uint32_t k = Q & 7;
+                if (lane == 0) cl_mbar_expect(&S.mb_dat[k], A * 32);
+                cl_mbar_wait(&S.mb_dat[k], (phase[k] & 1u));
+                phase[k] ^= 1u;
+                const uint64_t g0 = warp_sum61(lane < A ? S.inbox[k][lane][0] : 0), g1 = warp_sum61(lane < A ? S.inbox[k][lane][1] : 0);
+                const uint64_t g2 = warp_sum61(lane < A ? S.inbox[k][lane][2] : 0);
+                if (lane < 3) tr[3 * jj + lane] = lane == 0 ? g0 : (lane == 1 ? g1 : g2);
+                if (layer == 0 && jj == 0) {
+                    const uint64_t g3 = warp_sum61(lane < A ? S.inbox[k][lane][3] : 0);
+                    if (lane == 0) a.st->G[3] = g3;
+                }
+                __syncwarp();
+                if (lane == 0) S.tr_done = Q + 1;
+            }
+        }
+        tr += 7 * (size_t)s + 1;
+    }
+}
+
+// The two-level eq table of r1 (S.eqlo over variables 0..6, S.eqhi over 7..s-1), grown by one variable per challenge:
+// E[u + 2^k'] = E[u] r, E[u] -= E[u + 2^k'] for u < 2^k', k' = k mod 7 (one multiply per new entry).  Fold threads only;
+// consecutive steps are separated by the round barriers.
+__device__ __forceinline__ void cl_eq_step(ClShared &S, uint32_t k, uint64_t r, uint32_t ft, uint32_t nft) {
+    uint64_t *E = k < 7 ? S.eqlo : S.eqhi;
+    const uint32_t kk = k < 7 ? k : k - 7, half = 1u << kk;
+    for (uint32_t u = ft; u < half; u += nft) {
+        const uint64_t e = kk == 0 ? 1 : E[u], hi = fp61::mul(e, r);
+        E[u + half] = hi;
+        E[u] = fp61::sub(e, hi);
+    }
+}
+
+// What a layer needs from global memory before its first round: the level-0 slices of both phases (cp.async into shared
+// memory) and, per gate thread, its record and fixed operand (registers).  None of it depends on a challenge, so the
+// loads of layer i+1 are issued while layer i finishes (tau, z, claim), or while a joining CTA waits for the state.
+struct ClPre { uint32_t layer, i1, i2, t; uint64_t other; };
+__device__ __forceinline__ void cl_cp16(void *dst_smem, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(cl_smem(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cl_fetch(const ClArgs &a, const ClShared &S, uint8_t *dyn, uint32_t layer, uint32_t rank, ClPre &pre) {
+    const uint32_t tid = threadIdx.x;
+    constexpr uint32_t NM = CL_T - 64;
+    const ClPlanS &P = S.pl[layer - a.begin];
+    const ClLayer &C = P.C;
+    uint64_t *X = reinterpret_cast<uint64_t *>(dyn);
+    const uint32_t mmax = C.m[0] > C.m[1] ? C.m[0] : C.m[1];
+    uint64_t *Y = X + ((1u << mmax) < 64u ? 64u : (1u << mmax));
+    uint64_t *X2 = Y + ((1u << (mmax - 1)) < 64u ? 64u : (1u << (mmax - 1)));
+    {
+        const uint64_t *src = P.Vb + ((size_t)C.blk[0][rank] << C.m[0]);
+#pragma unroll 1
+        for (uint32_t v = tid; v < (1u << (C.m[0] - 1)); v += NM) cl_cp16(X + 2 * v, src + 2 * v);
+        src = P.Vb + ((size_t)C.blk[1][rank] << C.m[1]);
+#pragma unroll 1
+        for (uint32_t v = tid; v < (1u << (C.m[1] - 1)); v += NM) cl_cp16(X2 + 2 * v, src + 2 * v);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    pre.layer = layer; pre.i1 = 0; pre.i2 = 0; pre.t = VC_RELAY; pre.other = 0;
+    if (tid < C.gpc) {
+        Wires(P.Lp).get(rank * C.gpc + tid, pre.i1, pre.i2, pre.t);
+        pre.other = __ldg(P.Vb + pre.i2);
+    }
+}
+
+// ---- the rounds of one layer in an active CTA, gate threads (tid < ngt) and fold threads (256 <= tid < 256 + nft).
+// A gate thread's stream per round is: read the challenge, one multiply for the weight, wait for the level, read its
+// pair, two products, commit.  The fold threads build the level meanwhile and one of them (the dealer) draws the next
+// challenge while the gates form their products; the value is read by anyone only after the round's hand-off.
+__device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t *dyn, uint32_t layer, uint32_t rank, uint32_t Rb,
+                                          ClPhases &php, const ClPre &pre) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const LayerPlan &Lp = a.L[layer];
-    const ClLayer &C = a.cl[layer];
-    const uint32_t si = Lp.log_n, s = a.L[layer + 1].log_n, A = C.A, gpc = C.gpc, nact = C.nact;
-    const bool svc = warp == (CL_GT + CL_LT) / 32, has_ign = Lp.has_relay != 0;
-    const uint64_t *__restrict__ Vb = a.L[layer + 1].V;
+    const LayerPlan &Lp = S.pl[layer - a.begin].Lp;
+    const ClLayer &C = S.pl[layer - a.begin].C;
+    const uint32_t si = Lp.log_n, s = S.pl[layer - a.begin].s, A = C.A, gpc = C.gpc, ngt = C.ngt, nft = C.nft, np = ngt + nft;
+    const bool gate_thr = tid < CL_GW, has_ign = Lp.has_relay != 0;
+    const uint32_t ft = tid - CL_GW;                         // fold thread number (fold threads only)
+    const uint32_t pidx = gate_thr ? tid : ngt + ft;         // number among the np participants
+    const uint64_t *__restrict__ Vb = S.pl[layer - a.begin].Vb;
     FusedCtx &cx = S.cx;
     const uint64_t seed = cx.seed;
     const uint32_t ctr0 = (uint32_t)cx.ctr;
     const uint32_t arr_cnt = CL_C / A;                       // every active CTA contributes 16/A of the 16 arrivals
-    const bool live = !svc && tid < gpc;
+    const bool live = gate_thr && tid < gpc;
     const uint32_t g = rank * gpc + (live ? tid : 0);
-    const uint32_t ngw = (gpc + 31) >> 5;                    // warps that own gates
-    uint64_t *X = reinterpret_cast<uint64_t *>(dyn);
+    uint64_t *X = reinterpret_cast<uint64_t *>(dyn);          // level 0 of phase 1, then the even levels of both phases
     const uint32_t mmax = C.m[0] > C.m[1] ? C.m[0] : C.m[1];
-    uint64_t *Y = X + ((1u << mmax) < 64u ? 64u : (1u << mmax));
+    uint64_t *Y = X + ((1u << mmax) < 64u ? 64u : (1u << mmax));          // the odd levels
+    uint64_t *X2 = Y + ((1u << (mmax - 1)) < 64u ? 64u : (1u << (mmax - 1)));   // level 0 of phase 2, fetched while phase 1 runs
 #ifdef VC_TRACE
     const bool trace_thread = rank == 0 && tid == 0;
     uint32_t trow[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
 
-    // ---- a3 and the phase-1 state of this thread's gate
-    uint32_t i1 = 0, i2 = 0, t = VC_RELAY, idx = 0;
-    uint64_t W = 0, cP = fp61::P, P = 0, other = 0;
-    if (!svc) {
-        {   // level-0 slice of phase 1 first: the loads travel while the records are read and beta is built
-            const uint32_t m = C.m[0];
-            const ulonglong2 *src = reinterpret_cast<const ulonglong2 *>(Vb + ((size_t)C.blk[0][rank] << m));
+    // ---- a3 and the phase-1 state of this thread's gate (record, fixed operand and slices were fetched ahead: cl_fetch)
+    const uint32_t i1 = pre.i1, i2 = pre.i2, t = pre.t;
+    uint32_t idx = 0;
+    uint64_t W = 0, cP = fp61::P, P = 0;
+    const uint64_t other = pre.other;
+    CL_TRC(0);
+    if (si <= 6) {
+        if (live) P = eq_direct(g, cx.z, 0, si);
+    } else {
+        const uint32_t nl = 7, nh = si - 7;
 #pragma unroll 1
-            for (uint32_t v = tid; v < (1u << (m - 1)); v += nact) reinterpret_cast<ulonglong2 *>(X)[v] = __ldg(src + v);
+        for (uint32_t e = pidx; e < 128 + (1u << nh); e += np) {
+            if (e < 128) S.eqlo[e] = eq_direct(e, cx.z, 0, nl);
+            else S.eqhi[e - 128] = eq_direct(e - 128, cx.z, nl, si);
         }
-        if (live) {
-            Wires(Lp).get(g, i1, i2, t);
-            other = __ldg(Vb + i2);
-        }
-        if (si <= 6) {
-            if (live) P = eq_direct(g, cx.z, 0, si);
-        } else {
-            const uint32_t nl = 7, nh = si - 7;
-            if (tid < 128) S.eqlo[tid] = eq_direct(tid, cx.z, 0, nl);
-            else if (tid < 128 + (1u << nh)) S.eqhi[tid - 128] = eq_direct(tid - 128, cx.z, nl, si);
-            cl_bar(2, nact);
-            if (live) P = fp61::mul(S.eqlo[g & 127u], S.eqhi[g >> 7]);
-        }
-        if (live) {
-            uint64_t c; uint32_t ign;
-            gate_state(1, t, P, other, W, c, ign);
-            cP = c + fp61::P; idx = i1;
-        }
-        if (layer == 0) {                                    // a2: this CTA's share of the start claim V~_0(z_0)
-            const uint64_t part = warp_sum61(live ? fp61::mul(P, __ldg(Lp.V + g)) : 0);
-            if (lane == 0) cx.red[warp] = part;
-        }
-    } else if (lane <= s) {                                  // the service warp prepares the Lagrange denominators of the finish
-        const uint64_t dkv = fp61::mul(S.invfact[lane], S.invfact[s - lane]);
-        S.dk[lane] = ((s - lane) & 1u) ? fp61::neg(dkv) : dkv;
+        cl_bar(2, np);
+        if (live) P = fp61::mul(S.eqlo[g & 127u], S.eqhi[g >> 7]);
     }
-
-    if (svc) {
-        // ---- a5, one message behind the gates: this CTA's sums of message jj go to CTA 0's inbox (A > 1) or straight to the
-        // transcript (A = 1).  The service warp follows the hand-offs through rounds_done and frees the commit buffers
-        // through svc_done; it is on nobody's critical path.
-#pragma unroll 1
-        for (uint32_t jj = 0; jj < 2 * s; jj++) {
-#ifdef VC_TRACE
-            const uint32_t c_a = (uint32_t)clock64();
-#endif
-            while (S.rounds_done < jj + 1) __nanosleep(20);
-#ifdef VC_TRACE
-            const uint32_t c_b = (uint32_t)clock64();
-#endif
-            uint64_t t0, t1, t2;
-            cl_svc_sums(S.cbuf[jj & 3], gpc, t0, t1, t2);
-            if (lane == 0) S.svc_done = jj + 1;
-#ifdef VC_TRACE
-            const uint32_t c_c = (uint32_t)clock64();
-#endif
-            uint64_t t3 = 0;
-            if (layer == 0 && jj == 0) t3 = warp_sum61(lane < ngw ? cx.red[lane] : 0);
-            const uint64_t mine = lane == 0 ? t0 : (lane == 1 ? t1 : (lane == 2 ? t2 : t3));
-            if (A == 1) {                                    // the CTA's sums are the message
-                if (lane < 3) tr[3 * jj + lane] = mine;
-                if (layer == 0 && jj == 0 && lane == 3) cx.claim = mine;
-            } else {
-                if (rank == 0 && lane == 0) cl_mbar_expect(&S.mb_dat[jj & 7], A * 32);
-                if (lane < 4)
-                    cl_st_async(cl_mapa(cl_smem(&S.inbox[jj & 7][rank][lane]), 0), mine, cl_mapa(cl_smem(&S.mb_dat[jj & 7]), 0));
-                if (rank == 0 && jj >= 1) {                  // message jj-1: wait for its A shares, add them up, write the transcript
-                    const uint32_t k = (jj - 1) & 7;
-                    cl_mbar_wait(&S.mb_dat[k], php.dat[k]);
-                    php.dat[k] ^= 1u;
-                    const uint64_t g0 = warp_sum61(lane < A ? S.inbox[k][lane][0] : 0), g1 = warp_sum61(lane < A ? S.inbox[k][lane][1] : 0);
-                    const uint64_t g2 = warp_sum61(lane < A ? S.inbox[k][lane][2] : 0);
-                    if (lane < 3) tr[3 * (jj - 1) + lane] = lane == 0 ? g0 : (lane == 1 ? g1 : g2);
-                    if (layer == 0 && jj == 1) {
-                        const uint64_t g3 = warp_sum61(lane < A ? S.inbox[k][lane][3] : 0);
-                        if (lane == 0) cx.claim = g3;
-                    }
-                }
-            }
-#ifdef VC_TRACE
-            if (rank == 0 && lane == 0) {
-                uint32_t *row = S.trc2[jj < 64 ? jj : 63];
-                row[0] = c_a; row[1] = c_b; row[2] = c_c; row[3] = (uint32_t)clock64();
-            }
-#endif
-        }
-#ifdef VC_TRACE
-        if (rank == 0 && lane == 0) {
-            uint32_t *out = reinterpret_cast<uint32_t *>(a.stamps + a.d + 1) + 8 + 768 * 8 + layer * 64 * 4;
-            for (uint32_t q = 0; q < 2 * s && q < 64; q++) for (int e = 0; e < 4; e++) out[q * 4 + e] = S.trc2[q][e];
-        }
-#endif
-        if (rank == 0 && A > 1) {                            // the last message of the layer
-            const uint32_t k = (2 * s - 1) & 7;
-            cl_mbar_wait(&S.mb_dat[k], php.dat[k]);
-            php.dat[k] ^= 1u;
-            const uint64_t g0 = warp_sum61(lane < A ? S.inbox[k][lane][0] : 0), g1 = warp_sum61(lane < A ? S.inbox[k][lane][1] : 0);
-            const uint64_t g2 = warp_sum61(lane < A ? S.inbox[k][lane][2] : 0);
-            if (lane < 3) tr[3 * (2 * s - 1) + lane] = lane == 0 ? g0 : (lane == 1 ? g1 : g2);
-        }
-        if (A > 1) { php.rd[0] ^= s & 1u; php.rd[1] ^= s & 1u; }
-        if (C.m[0] < s) php.gat[0] ^= 1u;
-        if (C.m[1] < s) php.gat[1] ^= 1u;
-        return;
+    CL_TRC(1);
+    if (live) {
+        uint64_t c; uint32_t ign;
+        gate_state(1, t, P, other, W, c, ign);
+        cP = c + fp61::P; idx = i1;
+    }
+    CL_TRC(2);
+    if (layer == 0 && gate_thr) {                            // a2: this CTA's share of the start claim V~_0(z_0)
+        const uint64_t part = warp_sum61(live ? fp61::mul(P, __ldg(Lp.V + g)) : 0);
+        if (lane == 0) cx.red[warp] = part;
     }
 
     uint32_t jj = 0;                                         // round number within the layer, 0 .. 2s-1
-    uint64_t r_prev = 0;
     for (int ph = 0; ph < 2; ph++) {
         const uint32_t m = C.m[ph], blk = C.blk[ph][rank];
         const bool sliced = m < s;
         if (sliced && tid == 0) cl_mbar_expect(&S.mb_gat[ph], 2 * A * 8);
         if (ph == 1) {
+            CL_TRC_ROW(1000u * layer + 901u);
+            CL_TRC(0);
             // ---- phase switch: V~(r1) from the last level, P = beta(z,g) eq(in1[g], r1) through a two-level eq table of r1,
             // the phase-2 state, the new slice
-            const uint64_t *t1 = s == 1 ? X : (((s - 1) & 1) ? Y : X);
-            const uint64_t v1 = fold2(t1[0], t1[1], r_prev);
+            const uint64_t *t1 = s == 1 ? X : (((s - 1) & 1) ? Y : X);     // the last level of phase 1
+            const uint64_t v1 = fold2(t1[0], t1[1], S.chal[(jj - 1) & 1][0]);
             if (tid == 0) cx.v1 = v1;
-            {
-                const uint32_t nl = s < 7 ? s : 7, nh = s - nl, nlo = 1u << nl, ntot = nlo + (nh ? 1u << nh : 0u);
-#pragma unroll 1
-                for (uint32_t e = tid; e < ntot; e += nact) {
-                    const uint32_t hi = e >= nlo, u = hi ? e - nlo : e, k0 = hi ? nl : 0, k1 = hi ? s : nl;
-                    uint64_t e0 = 1, e1 = 1;                 // eq(u, r1[k0..k1)): two interleaved chains over the drawn challenges
-                    for (uint32_t k = k0; k < k1; k += 2) {
-                        const uint64_t ra = fp61::draw(seed, ctr0 + k);
-                        e0 = fp61::mul(e0, ((u >> (k - k0)) & 1u) ? ra : fp61::sub(1, ra));
-                        if (k + 1 < k1) {
-                            const uint64_t rb = fp61::draw(seed, ctr0 + k + 1);
-                            e1 = fp61::mul(e1, ((u >> (k + 1 - k0)) & 1u) ? rb : fp61::sub(1, rb));
-                        }
-                    }
-                    (hi ? S.eqhi : S.eqlo)[u] = fp61::mul(e0, e1);
-                }
-            }
-            cl_bar(2, nact);                                 // everyone has read the last level of phase 1; the eq table of r1 is complete
+            if (!gate_thr) cl_eq_step(S, s - 1, S.chal[(jj - 1) & 1][0], ft, nft);   // the last variable of the eq table of r1
+            CL_TRC(1);
+            cl_bar(2, np);                                   // everyone has read the last level of phase 1; the eq table of r1 is complete
+            CL_TRC(2);
             if (live) {
                 const uint32_t nl = s < 7 ? s : 7;
                 const uint64_t e1 = s > nl ? fp61::mul(S.eqlo[i1 & ((1u << nl) - 1)], S.eqhi[i1 >> nl]) : S.eqlo[i1];
@@ -339,64 +379,78 @@ __device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t 
                 gate_state(2, t, P, v1, W, c, ign);
                 cP = c + fp61::P; idx = i2 | (ign << 31);
             }
-            const ulonglong2 *src = reinterpret_cast<const ulonglong2 *>(Vb + ((size_t)blk << m));
-#pragma unroll 1
-            for (uint32_t v = tid; v < (1u << (m - 1)); v += nact) reinterpret_cast<ulonglong2 *>(X)[v] = __ldg(src + v);
         }
-        cl_bar(2, nact);                                     // level 0 is in place
+        CL_TRC(3);
+        if (ph == 0) asm volatile("cp.async.wait_all;" ::: "memory");
+        cl_bar(2, np);                                       // level 0 is in place
+        CL_TRC(4);
+        CL_TRC_ROW(1000u * layer + 900u + 2u * ph);
         CL_TRC(0);
 #pragma unroll 1
         for (uint32_t j = 0; j < s; j++, jj++) {
             const uint32_t par = jj & 1;
-            const uint64_t *tab = X;                         // level j as this CTA holds it
-            if (j >= 1) {
-                // ---- a6 for the challenge of the previous round: weight update, then level j of the fold table
-                if (live) W = fp61::mul(W, ((idx >> (j - 1)) & 1u) ? r_prev : fp61::sub(1, r_prev));
-                uint64_t *dst = (j & 1) ? Y : X;
-                const uint64_t *srcl = ((j - 1) & 1) ? Y : X;
-                if (sliced && j == m) {                      // the first whole level comes from the gathered level m-1
-                    cl_mbar_wait(&S.mb_gat[ph], php.gat[ph]);
-                    srcl = S.gat[ph];
+            const uint64_t *L0 = ph ? X2 : X;
+            const uint64_t *tab = j == 0 ? L0 : ((j & 1) ? Y : X);   // level j as this CTA holds it
+            if (gate_thr) {
+                if (j >= 1) {
+                    // ---- a6 for the challenge of the previous round: this gate's weight
+                    const ulonglong2 ch = *reinterpret_cast<const ulonglong2 *>(S.chal[(jj - 1) & 1]);
+                    if (live) W = fp61::mul(W, ((idx >> (j - 1)) & 1u) ? ch.x : ch.y);
+                    cl_bar(2, np);                           // level j is complete
                 }
-                const uint32_t cnt = j < m ? 1u << (m - j) : 1u << (s - j);
+                CL_TRC(1);
+                if (sliced && j == m - 1 && tid < 2 * A)     // this block's last pair goes to every CTA's gather buffer
+                    cl_st_async(cl_mapa(cl_smem(&S.gat[ph][2 * blk + (tid & 1u)]), tid >> 1), tab[tid & 1u],
+                                cl_mapa(cl_smem(&S.mb_gat[ph]), tid >> 1));
+                // ---- a4: this thread's gate against level j
+                if (live) {
+                    const uint32_t bit = (idx >> j) & 1u, u = (idx & F_IDX_MASK) >> (j + 1);
+                    const uint32_t pos = j < m ? 2 * u - (blk << (m - j)) : 2 * u;
+                    const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(tab + pos);
+                    uint64_t lo = p.x, hi = p.y;
+                    if (has_ign && (idx >> 31)) { lo = 0; hi = 0; }
+                    const uint64_t mb = (bit ? hi : lo) + cP, m2 = 2 * hi + cP - lo;
+                    const uint64_t y = cl_mul_lazy(W, m2), yc = (y & fp61::P) + (y >> 61);      // < 2^61 + 8
+                    ulonglong2 o;
+                    o.x = cl_mul_lazy(W, mb) | ((uint64_t)bit << 63);
+                    o.y = bit ? 2 * yc : 2 * fp61::P - yc;   // chi(bit, 2) W (x_2 + c), unreduced
+                    while (S.svc_done + 4 < Rb + jj + 1) { }     // the ring slot is free (the service warp is rarely that far behind)
+                    S.cbuf[(Rb + jj) & 3][tid] = o;
+                }
+            } else {
+                if (j >= 1) {
+                    // ---- a6: level j of the fold table from level j-1 and the challenge of the previous round
+                    const uint64_t r_prev = S.chal[(jj - 1) & 1][0];
+                    uint64_t *dst = (j & 1) ? Y : X;
+                    const uint64_t *srcl = j == 1 ? L0 : (((j - 1) & 1) ? Y : X);
+                    if (sliced && j == m) {                  // the first whole level comes from the gathered level m-1
+                        cl_mbar_wait(&S.mb_gat[ph], php.gat[ph]);
+                        srcl = S.gat[ph];
+                    }
+                    const uint32_t cnt = j < m ? 1u << (m - j) : 1u << (s - j);
 #pragma unroll 1
-                for (uint32_t v = tid; v < cnt; v += nact) {
-                    const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(srcl + 2 * (size_t)v);
-                    dst[v] = fold2(p.x, p.y, r_prev);
+                    for (uint32_t v = ft; v < cnt; v += nft) {
+                        const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(srcl + 2 * (size_t)v);
+                        dst[v] = fold2(p.x, p.y, r_prev);
+                    }
+                    cl_bar(2, np);
+                    if (ph == 0) cl_eq_step(S, j - 1, r_prev, ft, nft);   // the eq table of r1 grows by variable j-1 while the gates form their products
                 }
-                tab = dst;
-                cl_bar(2, nact);
-            }
-            CL_TRC(1);
-            if (sliced && j == m - 1 && tid < 2 * A)         // this block's last pair goes to every CTA's gather buffer
-                cl_st_async(cl_mapa(cl_smem(&S.gat[ph][2 * blk + (tid & 1u)]), tid >> 1), tab[tid & 1u],
-                            cl_mapa(cl_smem(&S.mb_gat[ph]), tid >> 1));
-            // ---- a4: this thread's gate against level j
-            if (live) {
-                const uint32_t bit = (idx >> j) & 1u, u = (idx & F_IDX_MASK) >> (j + 1);
-                const uint32_t pos = j < m ? 2 * u - (blk << (m - j)) : 2 * u;
-                const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(tab + pos);
-                uint64_t lo = p.x, hi = p.y;
-                if (has_ign && (idx >> 31)) { lo = 0; hi = 0; }
-                const uint64_t mb = (bit ? hi : lo) + cP, m2 = 2 * hi + cP - lo;
-                ulonglong2 o;
-                o.x = cl_mul_lazy(W, mb) | ((uint64_t)bit << 63);
-                o.y = cl_mul_lazy(W, m2);
-                if (jj >= 4) while (S.svc_done + 4 < jj + 1) { }   // the ring slot is free (the service warp is rarely that far behind)
-                S.cbuf[jj & 3][tid] = o;
+                if (ft == 0) {                               // the dealer: challenge jj, ready in shared memory before the commit barrier
+                    const uint64_t r = fp61::draw(seed, ctr0 + jj);
+                    ulonglong2 ch; ch.x = r; ch.y = fp61::sub(1, r);
+                    *reinterpret_cast<ulonglong2 *>(S.chal[par]) = ch;
+                }
             }
             CL_TRC(2);
-            cl_bar(3, nact);                                 // every contribution of this CTA to message jj is committed
+            cl_bar(3, np);                                   // every contribution of this CTA to message jj is committed
             CL_TRC(3);
-            if (A > 1 && warp == 0 && lane < A)
-                cl_mbar_arrive_remote(cl_mapa(cl_smem(&S.mb_rd[par]), lane), arr_cnt);
-            const uint64_t r = fp61::draw(seed, ctr0 + jj);   // the value is used only after the hand-off below
             if (A > 1) {
+                if (warp == 0 && lane < A) cl_mbar_arrive_remote(cl_mapa(cl_smem(&S.mb_rd[par]), lane), arr_cnt);
                 cl_mbar_wait_relaxed(&S.mb_rd[par], php.rd[par]);
                 php.rd[par] ^= 1u;
             }
-            r_prev = r;
-            if (tid == 0) S.rounds_done = jj + 1;            // the line and service warps may go on from here
+            if (tid == 0) S.rounds_done = Rb + jj + 1;       // the line and service warps may go on from here
             CL_TRC(4);
             CL_TRC_ROW(1000u * layer + jj);
             CL_TRC(0);
@@ -405,8 +459,8 @@ __device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t 
     }
     // ---- V~_{i+1}(r2) from the last level
     if (tid == 0) {
-        const uint64_t *t1 = s == 1 ? X : (((s - 1) & 1) ? Y : X);
-        cx.v2 = fold2(t1[0], t1[1], r_prev);
+        const uint64_t *t1 = s == 1 ? X2 : (((s - 1) & 1) ? Y : X);    // the last level of phase 2
+        cx.v2 = fold2(t1[0], t1[1], S.chal[(jj - 1) & 1][0]);
     }
 }
 
@@ -414,20 +468,20 @@ __device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t 
 // of phase 2, and leave the block's weighted values q_c[t], t = 2..s, in cx.acc[t - 2].  (Reading c-5; the polynomial
 // tree is that of vc_fused_line.cuh: a level-k node is a polynomial of degree k in t.)
 __device__ __forceinline__ void cl_line_wait(const ClShared &S, uint32_t need) {
-    while (S.rounds_done < need) __nanosleep(20);
+    while (S.rounds_done < need) { }
 }
-__device__ __forceinline__ void cl_line_stream(const ClArgs &a, ClShared &S, uint8_t *dyn, uint32_t layer, uint32_t rank) {
+__device__ __forceinline__ void cl_line_stream(const ClArgs &a, ClShared &S, uint8_t *dyn, uint32_t layer, uint32_t rank, uint32_t Rb) {
     const uint32_t lt = threadIdx.x - CL_GT;                 // 0 .. CL_LT-1
-    const ClLayer &C = a.cl[layer];
-    const uint32_t s = a.L[layer + 1].log_n, sb = C.sb, m = s - 1;
+    const ClLayer &C = S.pl[layer - a.begin].C;
+    const uint32_t s = S.pl[layer - a.begin].s, sb = C.sb, m = s - 1;
     FusedCtx &cx = S.cx;
     const uint64_t seed = cx.seed;
     const uint32_t ctr0 = (uint32_t)cx.ctr;
-    const uint64_t *__restrict__ Vblk = a.L[layer + 1].V + ((size_t)rank << sb);
+    const uint64_t *__restrict__ Vblk = S.pl[layer - a.begin].Vb + ((size_t)rank << sb);
     uint64_t *LA = reinterpret_cast<uint64_t *>(dyn + C.off_line);
     if (C.lmode == CL_LINE_DIRECT) {
         // tiny blocks (fewer than 8 words): q_c[t] = sum_u eq(u, l(t)) V[u] by direct products, once every challenge is known
-        cl_line_wait(S, 2 * s);
+        cl_line_wait(S, Rb + 2 * s);
         if (lt < m) {
             const uint32_t t = lt + 2;
             uint64_t acc = 0;
@@ -454,7 +508,7 @@ __device__ __forceinline__ void cl_line_stream(const ClArgs &a, ClShared &S, uin
 #pragma unroll
         for (int e = 0; e < 4; e++) w8[e] = __ldg(p2 + e);
     }
-    cl_line_wait(S, s + 3);                                  // r2_0..2 have been handed off
+    cl_line_wait(S, Rb + s + 3);                             // r2_0..2 have been handed off
     uint64_t x[3][4];
 #pragma unroll
     for (int k = 0; k < 3; k++) {
@@ -508,7 +562,7 @@ __device__ __forceinline__ void cl_line_stream(const ClArgs &a, ClShared &S, uin
     uint32_t ne = nE;
 #pragma unroll 1
     for (uint32_t k = 3; k < s; k++) {
-        cl_line_wait(S, s + k + 1);                          // r2_k has been handed off
+        cl_line_wait(S, Rb + s + k + 1);                     // r2_k has been handed off
         if (lt < m) {                                        // l(t)_k, t = 2..s
             const uint64_t p = fp61::draw(seed, ctr0 + k), q = fp61::draw(seed, ctr0 + s + k);
             S.lpts[lt] = fp61::add(p, fp61::mul(lt + 2, fp61::sub(q, p)));
@@ -570,12 +624,21 @@ __global__ void __launch_bounds__(CL_T, 1) k_cluster(ClArgs a) {
     uint8_t *dyn = cl_smem_raw + ((sizeof(ClShared) + 15) & ~(size_t)15);
     FusedCtx &cx = S.cx;
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, rank = cl_rank();
-    const bool svc = warp == (CL_GT + CL_LT) / 32, linew = tid >= CL_GT && !svc;
+    const bool linew = tid >= CL_GT && tid < CL_GT + CL_LT, trw = warp == (CL_GT + CL_LT) / 32, svc = warp == (CL_GT + CL_LT) / 32 + 1;
 #ifdef VC_TRACE
     const bool trace_thread = rank == 0 && tid == 0;
     uint32_t trow[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     if (tid == 0 && rank == 0) { g_tr_stamps = a.stamps; g_tr_d = a.d; S.trn = 0; }
 #endif
+    {   // the plans of this launch's layers: one read from global memory, at the start
+        const uint32_t nl = a.end - a.begin;
+        constexpr uint32_t WC = sizeof(ClLayer) / 4, WL = sizeof(LayerPlan) / 4;
+        for (uint32_t i = tid; i < nl * WC; i += CL_T)
+            reinterpret_cast<uint32_t *>(&S.pl[i / WC].C)[i % WC] = reinterpret_cast<const uint32_t *>(a.cl + a.begin + i / WC)[i % WC];
+        for (uint32_t i = tid; i < nl * WL; i += CL_T)
+            reinterpret_cast<uint32_t *>(&S.pl[i / WL].Lp)[i % WL] = reinterpret_cast<const uint32_t *>(a.L + a.begin + i / WL)[i % WL];
+        if (tid < nl) { S.pl[tid].Vb = a.L[a.begin + tid + 1].V; S.pl[tid].s = a.L[a.begin + tid + 1].log_n; }
+    }
     if (a.begin == 0) {
         const uint32_t s0 = a.L[0].log_n;
         if (tid < s0) cx.z[tid] = fp61::draw(a.seed, tid);           // a2: z_0
@@ -595,81 +658,100 @@ __global__ void __launch_bounds__(CL_T, 1) k_cluster(ClArgs a) {
         cl_mbar_init(&S.mb_state, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (tid == 0) { S.rounds_done = 0; S.svc_done = 0; S.tr_done = 0; }
     __syncthreads();
     cl_sync_all();                                               // every CTA's mbarriers exist before anyone arrives on them
-    uint64_t *tr = a.tr;
-    ClPhases php = {{0, 0}, {0, 0}, {0, 0, 0, 0, 0, 0, 0, 0}, {0, 0}, 0};
-    for (uint32_t layer = a.begin; layer < a.end; layer++) {
-        const ClLayer &C = a.cl[layer];
-        const uint32_t s = a.L[layer + 1].log_n, A = C.A, lp = (layer - a.begin) & 1u;
-        if (rank < A) {
-            const uint32_t prevA = layer > a.begin ? a.cl[layer - 1].A : 0;
-            if (prevA && rank >= prevA) {                        // this CTA joins: (z, claim, ctr) come from CTA 0
-                if (tid == 0) cl_mbar_expect(&S.mb_state, (MAX_VARS + 2) * 8);
-                cl_mbar_wait(&S.mb_state, php.state);
-                php.state ^= 1u;
-                if (tid < MAX_VARS) cx.z[tid] = S.state_in[tid];
-                if (tid == 0) { cx.claim = S.state_in[MAX_VARS]; cx.ctr = S.state_in[MAX_VARS + 1]; }
-            }
-            if (tid == 0) { S.rounds_done = 0; S.svc_done = 0; }
-            __syncthreads();
-            if (rank == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
-            CL_TRC(0);
-            if (A > 1 && tid == 0) cl_mbar_expect(&S.mb_end[lp], A * (s - 1) * 8);
-            const uint32_t ctr0 = (uint32_t)cx.ctr;
-            if (tid < C.nact || svc) cl_rounds(a, S, dyn, layer, tr, rank, php);
-            else {
-                if (linew && (C.lmode == CL_LINE_STREAM || C.lmode == CL_LINE_DIRECT)) cl_line_stream(a, S, dyn, layer, rank);
-                // the mbarrier phases this CTA went through, for threads that sat the rounds out
-                if (A > 1) { php.rd[0] ^= s & 1u; php.rd[1] ^= s & 1u; }
-                if (C.m[0] < s) php.gat[0] ^= 1u;
-                if (C.m[1] < s) php.gat[1] ^= 1u;
-            }
-            __syncthreads();
-            CL_TRC(1);
-            if (C.lmode == CL_LINE_PASS) {                       // a7 as a separate pass (blocks too large to stream)
-                if (tid < 2 * s) {
-                    const uint64_t r = fp61::draw(cx.seed, ctr0 + tid);
-                    if (tid < s) cx.r1[tid] = r; else cx.r2[tid - s] = r;
+    if (svc) cl_svc_role(a, S, rank);
+    else if (trw) { if (rank == 0) cl_tr_role(a, S); }
+    else {
+        constexpr uint32_t NM = CL_T - 64;                       // the threads of the layer loop: everyone but the two pipeline warps
+        uint64_t *tr = a.tr;
+        ClPhases php = {{0, 0}, {0, 0}, {0, 0, 0, 0, 0, 0, 0, 0}, {0, 0}, 0};
+        uint32_t Rb = 0;
+        ClPre pre; pre.layer = 0xffffffffu; pre.i1 = pre.i2 = 0; pre.t = VC_RELAY; pre.other = 0;
+        for (uint32_t layer = a.begin; layer < a.end; layer++) {
+            const ClLayer &C = S.pl[layer - a.begin].C;
+            const uint32_t s = S.pl[layer - a.begin].s, A = C.A, lp = (layer - a.begin) & 1u;
+            if (rank < A) {
+                const uint32_t prevA = layer > a.begin ? S.pl[layer - 1 - a.begin].C.A : 0;
+                if (pre.layer != layer) cl_fetch(a, S, dyn, layer, rank, pre);   // first layer of the launch, or a CTA that joins
+                if (prevA && rank >= prevA) {                    // this CTA joins: (z, claim, ctr) come from CTA 0
+                    if (tid == 0) cl_mbar_expect(&S.mb_state, (MAX_VARS + 2) * 8);
+                    cl_mbar_wait(&S.mb_state, php.state);
+                    php.state ^= 1u;
+                    if (tid < MAX_VARS) cx.z[tid] = S.state_in[tid];
+                    if (tid == 0) { cx.claim = S.state_in[MAX_VARS]; cx.ctr = S.state_in[MAX_VARS + 1]; }
+                    cl_bar(5, NM);
                 }
-                __syncthreads();
-                if (tid < C.lthr) line_partials(a.L[layer + 1].V, s, cx, S.pas, reinterpret_cast<uint64_t *>(dyn), rank, A, tid, C.lthr, C.ltb);
-                __syncthreads();
-            }
-            CL_TRC(2);
-            if (A > 1) {                                         // the s-1 block values of every CTA go to all A CTAs
-                for (uint32_t i = tid; i < (s - 1) * A; i += CL_T) {
-                    const uint32_t peer = i / (s - 1), k = i - peer * (s - 1);
-                    cl_st_async(cl_mapa(cl_smem(&S.qin[lp][rank][k]), peer), cx.acc[k], cl_mapa(cl_smem(&S.mb_end[lp]), peer));
-                }
-                if (warp == 0) {
-                    cl_mbar_wait(&S.mb_end[lp], php.end[lp]);
-                    if (lane < s - 1) {
-                        uint64_t sum = 0;
-                        for (uint32_t c = 0; c < A; c++) sum = fp61::add(sum, S.qin[lp][c][lane]);
-                        cx.acc[lane] = sum;
+                if (rank == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
+                CL_TRC(0);
+                if (A > 1 && tid == 0) cl_mbar_expect(&S.mb_end[lp], A * (s - 1) * 8);
+                const uint32_t ctr0 = (uint32_t)cx.ctr;
+                const bool part = tid < C.ngt || (tid >= CL_GW && tid < CL_GW + C.nft);
+                if (part) cl_rounds(a, S, dyn, layer, rank, Rb, php, pre);
+                else {
+                    if (linew) {
+                        const uint32_t lt = tid - CL_GT;
+                        if (lt <= s) {                           // the Lagrange denominators of the finish
+                            const uint64_t dkv = fp61::mul(S.invfact[lt], S.invfact[s - lt]);
+                            S.dk[lt] = ((s - lt) & 1u) ? fp61::neg(dkv) : dkv;
+                        }
+                        if (C.lmode == CL_LINE_STREAM || C.lmode == CL_LINE_DIRECT) cl_line_stream(a, S, dyn, layer, rank, Rb);
                     }
-                    __syncwarp();
+                    // the mbarrier phases this CTA went through, for threads that sat the rounds out
+                    if (A > 1) { php.rd[0] ^= s & 1u; php.rd[1] ^= s & 1u; }
+                    if (C.m[0] < s) php.gat[0] ^= 1u;
+                    if (C.m[1] < s) php.gat[1] ^= 1u;
                 }
-                php.end[lp] ^= 1u;
-            }
-            CL_TRC(3);
-            if (warp == 0) cl_finish(s, S, ctr0, tr + 6 * (size_t)s, rank == 0);
-            __syncthreads();
-            if (rank == 0 && layer + 1 < a.end && a.cl[layer + 1].A > A) {   // wider layer next: hand the state to the CTAs that join
-                const uint32_t An = a.cl[layer + 1].A;
-                for (uint32_t i = tid; i < (An - A) * (MAX_VARS + 2); i += CL_T) {
-                    const uint32_t peer = A + i / (MAX_VARS + 2), k = i % (MAX_VARS + 2);
-                    const uint64_t v = k < MAX_VARS ? cx.z[k] : (k == MAX_VARS ? cx.claim : cx.ctr);
-                    cl_st_async(cl_mapa(cl_smem(&S.state_in[k]), peer), v, cl_mapa(cl_smem(&S.mb_state), peer));
+                Rb += 2 * s;
+                CL_TRC(1);
+                cl_bar(5, NM);
+                CL_TRC(2);
+                if (C.lmode == CL_LINE_PASS) {                   // a7 as a separate pass (blocks too large to stream)
+                    if (tid < 2 * s) {
+                        const uint64_t r = fp61::draw(cx.seed, ctr0 + tid);
+                        if (tid < s) cx.r1[tid] = r; else cx.r2[tid - s] = r;
+                    }
+                    cl_bar(5, NM);
+                    if (tid < C.lthr) line_partials(S.pl[layer - a.begin].Vb, s, cx, S.pas, reinterpret_cast<uint64_t *>(dyn), rank, A, tid, C.lthr, C.ltb);
+                    cl_bar(5, NM);
                 }
+                if (layer + 1 < a.end && rank < S.pl[layer + 1 - a.begin].C.A) cl_fetch(a, S, dyn, layer + 1, rank, pre);   // the next layer's loads travel during the finish
+                if (A > 1) {                                     // the s-1 block values of every CTA go to all A CTAs
+                    for (uint32_t i = tid; i < (s - 1) * A; i += NM) {
+                        const uint32_t peer = i / (s - 1), k = i - peer * (s - 1);
+                        cl_st_async(cl_mapa(cl_smem(&S.qin[lp][rank][k]), peer), cx.acc[k], cl_mapa(cl_smem(&S.mb_end[lp]), peer));
+                    }
+                    if (warp == 0) {
+                        cl_mbar_wait(&S.mb_end[lp], php.end[lp]);
+                        if (lane < s - 1) {
+                            uint64_t sum = 0;
+                            for (uint32_t c = 0; c < A; c++) sum = fp61::add(sum, S.qin[lp][c][lane]);
+                            cx.acc[lane] = sum;
+                        }
+                        __syncwarp();
+                    }
+                    php.end[lp] ^= 1u;
+                }
+                CL_TRC(3);
+                if (warp == 0) cl_finish(s, S, ctr0, tr + 6 * (size_t)s, rank == 0);
+                cl_bar(5, NM);
+                if (rank == 0 && layer + 1 < a.end && S.pl[layer + 1 - a.begin].C.A > A) {   // wider layer next: hand the state to the CTAs that join
+                    const uint32_t An = S.pl[layer + 1 - a.begin].C.A;
+                    for (uint32_t i = tid; i < (An - A) * (MAX_VARS + 2); i += NM) {
+                        const uint32_t peer = A + i / (MAX_VARS + 2), k = i % (MAX_VARS + 2);
+                        const uint64_t v = k < MAX_VARS ? cx.z[k] : (k == MAX_VARS ? cx.claim : cx.ctr);
+                        cl_st_async(cl_mapa(cl_smem(&S.state_in[k]), peer), v, cl_mapa(cl_smem(&S.mb_state), peer));
+                    }
+                }
+                CL_TRC(4);
+                CL_TRC_ROW(1000u * layer + 999u);
             }
-            CL_TRC(4);
-            CL_TRC_ROW(1000u * layer + 999u);
+            tr += 7 * (size_t)s + 1;
         }
-        tr += 7 * (size_t)s + 1;
     }
     if (rank == 0 && tid == 0) a.stamps[a.end] = globaltimer_ns();
+    __syncthreads();                                             // the pipeline warps have written the last transcript words
     if (rank == 0) {
         if (tid < MAX_VARS) a.st->z[tid] = cx.z[tid];
         if (tid == 0) { a.st->seed = cx.seed; a.st->ctr = cx.ctr; a.st->claim = cx.claim; a.st->bar_gen = cx.epoch; }

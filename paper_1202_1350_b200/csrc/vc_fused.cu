@@ -303,15 +303,15 @@ static size_t cl_line_words(uint32_t s, uint32_t tb) {
     return (((s + 1) * sp + 1) & ~(size_t)1) + NB * P + (NB * P + 1) / 2 + 1 + 64 + 8;
 }
 static bool plan_cluster_layer(const vc_circuit *c, uint32_t i, int csize, ClLayer &cl, size_t &dyn_bytes) {
-    static const int target_gpc = getenv("VC_CL_GPC") ? atoi(getenv("VC_CL_GPC")) : 256;
-    static const int single_max = getenv("VC_CL_SINGLE") ? atoi(getenv("VC_CL_SINGLE")) : 512;
+    static const int target_gpc = getenv("VC_CL_GPC") ? atoi(getenv("VC_CL_GPC")) : 128;
+    static const int single_max = getenv("VC_CL_SINGLE") ? atoi(getenv("VC_CL_SINGLE")) : 256;
     const uint32_t si = c->logs[i], s = c->logs[i + 1];
     cl = ClLayer{};
     if (si > CL_MAX_N || s > CL_MAX_S) return false;
     const uint32_t n = 1u << si;
     uint32_t A = 1;
     if ((int)n > single_max) { while (A < (uint32_t)csize && n / A > (uint32_t)target_gpc) A <<= 1; }
-    while (n / A > (uint32_t)CL_GT) { if (A >= (uint32_t)csize) return false; A <<= 1; }
+    while (n / A > (uint32_t)CL_GW) { if (A >= (uint32_t)csize) return false; A <<= 1; }
     if (A > n) A = n;
     const uint32_t gpc = n / A;
     uint32_t mmax = 1;
@@ -337,13 +337,15 @@ static bool plan_cluster_layer(const vc_circuit *c, uint32_t i, int csize, ClLay
         mmax = std::max(mmax, m);
     }
     cl.A = A; cl.gpc = gpc;
-    uint32_t nact = std::max<uint32_t>(gpc, std::min<uint32_t>(CL_GT, 1u << (mmax - 1)));
-    if (si > 6) nact = std::max<uint32_t>(nact, 192);
-    cl.nact = std::min<uint32_t>(CL_GT, (nact + 31) & ~31u);
+    cl.ngt = (gpc + 31) & ~31u;
+    uint32_t nft = std::min<uint32_t>(CL_FW, std::max<uint32_t>(32, 1u << (mmax - 1)));
+    if (si > 6 && cl.ngt + nft < 192) nft = 192 - cl.ngt;
+    cl.nft = (nft + 31) & ~31u;
     uint32_t la = 0; while ((1u << la) < A) la++;
     if (s < la) return false;
     cl.sb = s - la;
-    const size_t tabw = std::max<size_t>((size_t)1 << mmax, 64) + std::max<size_t>((size_t)1 << (mmax - 1), 64);
+    const size_t tabw = std::max<size_t>((size_t)1 << mmax, 64) + std::max<size_t>((size_t)1 << (mmax - 1), 64) +
+                        std::max<size_t>((size_t)1 << cl.m[1], 64);       // X, Y and the phase-2 level 0
     cl.off_line = (uint32_t)(tabw * 8);
     size_t need = tabw * 8;
     cl.ltb = 0; cl.lthr = 32;
@@ -506,7 +508,7 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
     std::vector<std::pair<uint32_t, int>> runs;          // (first layer, mask)
     for (uint32_t i = begin; i < end; i++) {
         const int m = fh->group[i];
-        if (runs.empty() || runs.back().second != m) runs.emplace_back(i, m);
+        if (runs.empty() || runs.back().second != m || (m == 8 && i - runs.back().first >= CL_MAX_LAYERS)) runs.emplace_back(i, m);
     }
     if (runs.size() > F_MAX_RUNS || g_single_kernel) {   // the all-kinds kernel cannot hold cluster layers: they keep their own launches
         bool has_cl = false;
