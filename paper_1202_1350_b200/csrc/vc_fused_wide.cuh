@@ -138,6 +138,96 @@ __device__ __forceinline__ void hot_gates(const bool UPD, uint64_t *sW, const ui
     flush();
 }
 
+// ---- the resident hot loop for rounds j >= 1 of a sliced phase: table in shared memory, weight update pending.
+// Per gate-round: one multiply for the weight, two products into 128-bit accumulators, nothing else that is not a load
+// or an address.  Against hot_gates it drops (a) the canonical form of W between rounds: W' = W f is left below
+// 2^61 + 4 (w1 <= 2^29 keeps every partial product in range: p11 = w1 f1 < 2^58, mid = w0 f1 + w1 f0 < 2^62), and the
+// fold uses 2^61 = 1: W f = p00 + mid 2^32 + p11 2^64 = (p00 mod') + (mid >> 29) + (mid & (2^29-1)) 2^32 + 8 p11, with
+// 8 f1 formed once per gate from the selected f; (b) generic addressing: the table is addressed as shared memory;
+// (c) the accumulator flushes: products are < 2^61.01 * 2^63, fifteen of them fit 128 bits, so one flush per 14 gates.
+__device__ __forceinline__ uint64_t mul_wide(uint32_t a, uint32_t b) { uint64_t r; asm("mul.wide.u32 %0, %1, %2;" : "=l"(r) : "r"(a), "r"(b)); return r; }
+__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) { uint64_t r; asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c)); return r; }
+__device__ __forceinline__ uint64_t mul_lazy61(uint64_t W, uint32_t f0, uint32_t f1) {
+    const uint32_t w0 = (uint32_t)W, w1 = (uint32_t)(W >> 32), f1x8 = f1 << 3;
+    const uint64_t p00 = mul_wide(w0, f0);
+    const uint64_t mid = mad_wide(w1, f0, mul_wide(w0, f1));                              // < 2^62
+    uint64_t s = mad_wide(w1, f1x8, mid >> 29);                                             // 8 p11 + (mid >> 29) < 2^61 + 2^33
+    s = ((uint64_t)((uint32_t)(s >> 32) + ((uint32_t)mid & 0x1fffffffu)) << 32) | (uint32_t)s;   // + (mid & (2^29-1)) 2^32: high word only, < 2^62
+    s += (p00 & fp61::P) + (p00 >> 61);                                                     // < 2^63
+    return (s & fp61::P) + (s >> 61);                                                       // < 2^61 + 4
+}
+__device__ __forceinline__ ulonglong2 lds_pair(uint32_t saddr) {
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(saddr));
+    return v;
+}
+#ifndef VC_HOT_ILP
+#define VC_HOT_ILP 2
+#endif
+template <bool IGN>
+__device__ __forceinline__ void hot_gates_sm(uint64_t *sW, const uint64_t *sC, const uint32_t *sI, uint32_t tb_s, uint32_t j,
+                                             uint32_t nmine, uint32_t tid, uint64_t r_prev, uint64_t omr, uint64_t (&s4)[4]) {
+    constexpr uint32_t GT = FT, CHUNK = 14;
+    acc128 X0, X1, Y0, Y1; X0.clear(); X1.clear(); Y0.clear(); Y1.clear();
+    const uint32_t sh = j + 1;
+    const uint32_t r0 = (uint32_t)r_prev, r1 = (uint32_t)(r_prev >> 32), o0 = (uint32_t)omr, o1 = (uint32_t)(omr >> 32);
+    auto one = [&](uint64_t &W, uint64_t cP, uint32_t idx, const ulonglong2 pr) {
+        const bool bp = (idx >> (j - 1)) & 1u;
+        W = mul_lazy61(W, bp ? r0 : o0, bp ? r1 : o1);
+        uint64_t lo = pr.x, hi = pr.y;
+        if (IGN && (idx >> 31)) { lo = 0; hi = 0; }
+        const uint32_t bit = (idx >> j) & 1u;
+        const uint64_t mb = (bit ? hi : lo) + cP;                // < 2^61 + 2^62
+        const uint64_t m2 = 2 * hi + cP - lo;                    // 2 hi - lo + c + p  in (0, 2^63)
+        const uint64_t pl = W * mb, ph = fp61::mulhi(W, mb), ql = W * m2, qh = fp61::mulhi(W, m2);
+        if (bit) { mac1(X1, pl, ph); mac1(Y1, ql, qh); } else { mac1(X0, pl, ph); mac1(Y0, ql, qh); }
+    };
+    auto flush = [&]() {
+        s4[0] = fp61::add(s4[0], X0.value()); s4[1] = fp61::add(s4[1], X1.value());
+        s4[2] = fp61::add(s4[2], Y0.value()); s4[3] = fp61::add(s4[3], Y1.value());
+        X0.clear(); X1.clear(); Y0.clear(); Y1.clear();
+    };
+    uint32_t k = 0, inacc = 0;
+#if VC_HOT_ILP == 4
+    for (; k + 4 <= nmine; k += 4) {
+        const uint32_t l0 = k * GT + tid, l1 = l0 + GT, l2 = l1 + GT, l3 = l2 + GT;
+        uint64_t Wa = sW[l0], Wb = sW[l1], Wc = sW[l2], Wd = sW[l3];
+        const uint64_t ca = sC[l0], cb = sC[l1], cc = sC[l2], cd = sC[l3];
+        const uint32_t ia = sI[l0], ib = sI[l1], ic = sI[l2], id = sI[l3];
+        const ulonglong2 pa = lds_pair(tb_s + (((IGN ? ia & F_IDX_MASK : ia) >> sh) << 4));
+        const ulonglong2 pb = lds_pair(tb_s + (((IGN ? ib & F_IDX_MASK : ib) >> sh) << 4));
+        const ulonglong2 pc = lds_pair(tb_s + (((IGN ? ic & F_IDX_MASK : ic) >> sh) << 4));
+        const ulonglong2 pd = lds_pair(tb_s + (((IGN ? id & F_IDX_MASK : id) >> sh) << 4));
+        one(Wa, ca, ia, pa); one(Wb, cb, ib, pb); one(Wc, cc, ic, pc); one(Wd, cd, id, pd);
+        sW[l0] = Wa; sW[l1] = Wb; sW[l2] = Wc; sW[l3] = Wd;
+        inacc += 4;
+        if (inacc >= CHUNK - 2) { flush(); inacc = 0; }
+    }
+#endif
+    for (; k + 2 <= nmine; k += 2) {
+        const uint32_t l0 = k * GT + tid, l1 = l0 + GT;
+        uint64_t Wa = sW[l0], Wb = sW[l1];
+        const uint64_t ca = sC[l0], cb = sC[l1];
+        const uint32_t ia = sI[l0], ib = sI[l1];
+        const ulonglong2 pa = lds_pair(tb_s + (((IGN ? ia & F_IDX_MASK : ia) >> sh) << 4));
+        const ulonglong2 pb = lds_pair(tb_s + (((IGN ? ib & F_IDX_MASK : ib) >> sh) << 4));
+        one(Wa, ca, ia, pa);
+        one(Wb, cb, ib, pb);
+        sW[l0] = Wa; sW[l1] = Wb;
+        inacc += 2;
+        if (inacc >= CHUNK) { flush(); inacc = 0; }
+    }
+    if (k < nmine) {
+        const uint32_t l0 = k * GT + tid;
+        uint64_t Wa = sW[l0];
+        const uint32_t ia = sI[l0];
+        const ulonglong2 pa = lds_pair(tb_s + (((IGN ? ia & F_IDX_MASK : ia) >> sh) << 4));
+        one(Wa, sC[l0], ia, pa);
+        sW[l0] = Wa;
+    }
+    flush();
+}
+
 __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, const uint64_t *invfact, const uint32_t *pas, uint8_t *dyn,
                                            uint32_t layer, uint64_t *tr) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x, b = blockIdx.x;
@@ -293,7 +383,11 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                 uint64_t s4[4] = {0, 0, 0, 0};                 // canonical running sums of X, X1, Y, Y1 (flushed every 8 products)
                 if (res && mode == F_MODE_SLICE) {
                     // hot loop: state in shared memory; the table is level 0 in L2 (round 0) or a shared-memory buffer
-                    if (has_ign) hot_gates<true>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
+                    if (j >= 1) {                          // level j sits in shared memory and a weight update is pending: the slim loop
+                        const uint32_t tb_s = (uint32_t)__cvta_generic_to_shared(tab) - base * 8u;
+                        if (has_ign) hot_gates_sm<true>(sW, sC, sI, tb_s, j, nmine, tid, r_prev, omr, s4);
+                        else hot_gates_sm<false>(sW, sC, sI, tb_s, j, nmine, tid, r_prev, omr, s4);
+                    } else if (has_ign) hot_gates<true>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                     else hot_gates<false>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                 } else {
                     const Wires wr(Lp);
