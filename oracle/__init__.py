@@ -75,6 +75,8 @@ def lib():
         L.orc_transcript_words.argtypes = [vp, u32, u32]
         L.orc_prove.restype = C.c_int
         L.orc_prove.argtypes = [vp, u32, u32, vp, u64, vp, vp, u64, vp, vp]
+        L.orc_layer_entry.restype = u64
+        L.orc_layer_entry.argtypes = [vp, u32, u64, vp]
         L.orc_verify.restype = C.c_int
         L.orc_verify.argtypes = [vp, u32, u32, vp, vp, u64, vp, u64, vp, vp, vp]
         _lib = L
@@ -169,26 +171,12 @@ class OracleCircuit:
             raise ValueError(f"orc_verify rc={rc}")
         return bool(acc.value), int(fl.value), int(fr.value)
 
-    # -- entry state of a layer in isolation: challenges are counter-based (reading c-11), so the
-    #    claim point of layer i is a function of the draws alone; the claim is V~_i(z) by definition.
     def layer_entry(self, i, seed, Vi):
-        L = lib()
-        logs = [l.log_size for l in self.c.layers] + [self.log_input]
-        if i == 0:
-            z = [int(L.orc_draw(seed, k)) for k in range(logs[0])]
-            ctr = logs[0]
-        else:
-            c0 = logs[0] + sum(2 * logs[l + 1] + 1 for l in range(i - 1))
-            s = logs[i]
-            r1 = [int(L.orc_draw(seed, c0 + k)) for k in range(s)]
-            r2 = [int(L.orc_draw(seed, c0 + s + k)) for k in range(s)]
-            tau = int(L.orc_draw(seed, c0 + 2 * s))
-            z = [int(L.orc_add(a, L.orc_mul(tau, L.orc_sub(b, a)))) for a, b in zip(r1, r2)]
-            ctr = c0 + 2 * s + 1
+        """Entry state (z, claim, counter) of layer i in isolation: orc_layer_entry for the point, orc_mle for the claim."""
+        logs = np.array([l.log_size for l in self.c.layers] + [self.log_input], dtype=np.uint32)
         zz = np.zeros(64, dtype=np.uint64)
-        zz[:len(z)] = z
-        claim = mle(Vi, z)
-        return zz, claim, ctr
+        ctr = int(lib().orc_layer_entry(logs.ctypes.data_as(C.c_void_p), i, seed, _ptr(zz)))
+        return zz, mle(Vi, zz), ctr
 
 
 def mle(V, x) -> int:

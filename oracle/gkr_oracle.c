@@ -243,6 +243,27 @@ int orc_prove_layer(const orc_layer *L, uint32_t s, const uint64_t *Vb, uint64_t
     return ORC_OK;
 }
 
+/* Entry state of layer i taken in isolation.  The challenges are a function of (seed, counter) alone (reading c-11),
+ * the counter advances by s_0 for z_0 and by 2 s_{l+1} + 1 per proved layer l (2s round challenges, then tau), and
+ * the claim point of layer i >= 1 is z = l(tau) = r1 + tau (r2 - r1) with r1, r2, tau the draws of layer i-1
+ * (reading c-5).  logs[0..i] = log sizes of layers 0..i.  Writes z[0 .. logs[i]) and returns the counter at which
+ * layer i's own draws start.  (The claim at z is V~_i(z) by definition: orc_mle.) */
+uint64_t orc_layer_entry(const uint32_t *logs, uint32_t i, uint64_t seed, uint64_t *z) {
+    if (i == 0) {
+        for (uint32_t k = 0; k < logs[0]; k++) z[k] = orc_draw(seed, k);
+        return logs[0];
+    }
+    uint64_t c0 = logs[0];
+    for (uint32_t l = 0; l + 1 < i; l++) c0 += 2ull * logs[l + 1] + 1;
+    const uint32_t s = logs[i];
+    const uint64_t tau = orc_draw(seed, c0 + 2ull * s);
+    for (uint32_t k = 0; k < s; k++) {
+        const uint64_t r1 = orc_draw(seed, c0 + k), r2 = orc_draw(seed, c0 + s + k);
+        z[k] = orc_add(r1, orc_mul(tau, orc_sub(r2, r1)));
+    }
+    return c0 + 2ull * s + 1;
+}
+
 static uint32_t log_below(const orc_layer *layers, uint32_t d, uint32_t log_input, uint32_t i) {
     return i + 1 < d ? layers[i + 1].log_size : log_input;
 }
