@@ -45,8 +45,12 @@ int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_c
 
 /* vc_evaluate — layered circuit evaluation (step a1; §6.2.4):
  * V_d = input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]).
- *   d_input   DEVICE pointer, 2^log_input canonical words (read; a non-canonical word makes the
- *             next vc_prove_layer fail with VC_ERR_ARG once the flag is read back — see vc_status).
+ *   d_input   DEVICE pointer, 2^log_input canonical words (read).  A word >= p is detected ON THE DEVICE while the input
+ *             is copied, i.e. asynchronously: the call itself still returns VC_OK ("enqueued").  The sticky bit 0 of the
+ *             status word reports it for THIS evaluation (it is cleared when vc_evaluate is enqueued): vc_status reads
+ *             it after a stream synchronise, and vc_run_host, which synchronises anyway, returns VC_ERR_ARG.
+ *             (SURVEY.md §8(b) "Errors": non-canonical input -> VC_ERR_ARG at load or evaluate; detection cannot be
+ *             synchronous without a device round-trip inside a call that must not synchronise.)
  *   d_outputs DEVICE pointer, 2^log_size(layer 0) words (written); may be NULL.
  * Resets the proof state (next vc_prove_layer must be layer 0). */
 int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, void *cuda_stream);
@@ -118,7 +122,7 @@ int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, voi
 /* the device sums of the last vc_verify_transcript_device call on this circuit, n = 4 d + 2 HOST words:
  * [0] start claim, [1 + 4 i + t] wiring sum of type t of layer i, [1 + 4 d] the input extension at z_d */
 int vc_debug_verifier_sums(const vc_circuit *c, uint64_t *h_sums, uint64_t n);
-/* sticky device-side status: 0 = fine, 1 = a non-canonical input word was seen by vc_evaluate */
+/* device-side status of the last vc_evaluate on this handle: 0 = fine, bit 0 = a non-canonical input word was seen */
 int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */
 uint64_t vc_launch_count(void);
@@ -126,7 +130,8 @@ uint64_t vc_launch_count(void);
 int vc_set_schedule(vc_circuit *c, int schedule);
 
 /* Field/PRNG probes for the GPU unit tests: out[i] = op(a[i], b[i]) on the device, n words each,
- * all DEVICE pointers.  op: 0 add, 1 sub, 2 mul, 3 draw(seed=a[i], ctr=b[i]). */
+ * all DEVICE pointers.  op: 0 add, 1 sub, 2 mul, 3 draw(seed=a[i], ctr=b[i]), 4 sum of 64 products a[i]*b[i] through the
+ * lazy 128-bit accumulator (one fold at the end). */
 int vc_debug_fieldop(int op, const uint64_t *d_a, const uint64_t *d_b, uint64_t *d_out, uint64_t n,
                      void *cuda_stream);
 /* Integer-multiply roofline microbenchmark: runs `iters` dependent fp61 multiplies in each of `ilp`

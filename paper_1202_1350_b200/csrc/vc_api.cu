@@ -15,7 +15,8 @@ namespace vc {
 std::atomic<uint64_t> g_launches{0};
 bool g_profile = false;
 std::vector<ProfRec> g_prof;
-void prof_push(int kind, cudaEvent_t a, cudaEvent_t b) { g_prof.push_back({kind, a, b}); }
+std::mutex g_registry_mutex;
+void prof_push(int kind, cudaEvent_t a, cudaEvent_t b) { std::lock_guard<std::mutex> lk(g_registry_mutex); g_prof.push_back({kind, a, b}); }
 }
 
 #define CUDA_TRY(x)                                          \
@@ -63,7 +64,6 @@ extern "C" void vc_circuit_free(vc_circuit *c) {
     for (auto p : c->d_V) cudaFree(p);
     cudaFree(c->d_P); cudaFree(c->d_T0); cudaFree(c->d_T1); cudaFree(c->d_part); cudaFree(c->d_tr);
     cudaFree(c->d_state);
-    if (c->h_pin) cudaFreeHost(c->h_pin);
     delete c;
 }
 
@@ -124,8 +124,6 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
     CUDA_TRY(cudaMalloc(&c->d_part, part * 8));
     CUDA_TRY(cudaMalloc(&c->d_tr, total * 8));
     CUDA_TRY(cudaMalloc(&c->d_state, sizeof(vc::DevState)));
-    const size_t pin_words = ((size_t)1 << log_input) + ((size_t)1 << c->logs[0]) + total;
-    CUDA_TRY(cudaMallocHost(&c->h_pin, pin_words * 8));
     // proof state: zero, plus 1/k! for the Lagrange denominators (constants of the method, not data)
     vc::DevState *hs = new (std::nothrow) vc::DevState();
     if (!hs) return VC_ERR_NOMEM;
@@ -159,6 +157,7 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const uint32_t d = c->d;
     const uint64_t n_in = 1ull << c->log_input;
+    CUDA_TRY(cudaMemsetAsync(&c->d_state->flags, 0, sizeof(unsigned int), st));   // the status word reports THIS evaluation
     if (c->schedule != 1) {                      // one cooperative launch for the whole evaluation when the circuit allows it
         const int rc = vc::enqueue_eval_fused(c, d_input, d_outputs, st);
         if (rc == VC_OK) { c->next_layer = 0; return VC_OK; }
@@ -374,6 +373,7 @@ extern "C" int vc_bench_modmul(uint32_t grid, uint32_t block, uint32_t iters, ui
 
 // ------------------------------------------------------------------ per-kernel-kind timing for bench.py's roofline
 extern "C" int vc_profile_enable(int on) {
+    std::lock_guard<std::mutex> lk(vc::g_registry_mutex);
     for (auto &r : vc::g_prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     vc::g_prof.clear();
     vc::g_profile = on != 0;
@@ -382,6 +382,7 @@ extern "C" int vc_profile_enable(int on) {
 extern "C" int vc_profile_read(uint64_t *launches, double *ms) {
     if (!launches || !ms) return VC_ERR_ARG;
     CUDA_TRY(cudaDeviceSynchronize());
+    std::lock_guard<std::mutex> lk(vc::g_registry_mutex);
     for (int k = 0; k < VC_K_COUNT; k++) { launches[k] = 0; ms[k] = 0.0; }
     for (auto &r : vc::g_prof) {
         float t = 0.f;

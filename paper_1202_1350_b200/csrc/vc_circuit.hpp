@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include <atomic>
+#include <mutex>
 #include <vector>
 
 #include "../../include/vc.h"
@@ -28,7 +29,6 @@ struct vc_circuit {
     uint64_t *d_part = nullptr;                 // block partials
     uint64_t *d_tr = nullptr;                   // internal transcript buffer (vc_run_host)
     vc::DevState *d_state = nullptr;
-    uint64_t *h_pin = nullptr;                  // pinned staging for vc_run_host
     size_t part_words = 0;
     uint64_t total_words = 0;
     // proof sequencing
@@ -43,6 +43,7 @@ struct vc_circuit {
 
 namespace vc {
 extern std::atomic<uint64_t> g_launches;
+extern std::mutex g_registry_mutex;         // guards the process-wide registries (fused plans, verifier scratch, profile records)
 struct ProfRec { int kind; cudaEvent_t a, b; };
 extern bool g_profile;                      // vc_profile_enable: CUDA events around every launch, by kind
 void prof_push(int kind, cudaEvent_t a, cudaEvent_t b);

@@ -1,5 +1,6 @@
 // vc_fused.cu — kernel + host driver (load-time plan, launch) of the on-chip schedule (see vc_fused.cuh).
 #include <algorithm>
+#include <new>
 #include <cstdlib>
 #include <vector>
 
@@ -181,7 +182,6 @@ constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
 constexpr size_t F_MAX_RUNS = 8;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
-static bool g_single_kernel = false;               // VC_SINGLE_KERNEL=1 in the environment at load: always the all-kinds kernel (A/B measurements)
 
 struct FusedHost {
     LayerPlan *d_plan = nullptr;
@@ -195,12 +195,19 @@ struct FusedHost {
     size_t smem = 0;
     ClLayer *d_cl = nullptr;                       // the cluster engine's plans (vc_cluster.cuh)
     int csize = 0;                                 // CTAs per cluster (0: engine unavailable)
+    bool single_kernel = false;                    // VC_SINGLE_KERNEL=1 in the environment at load: always the all-kinds kernel (A/B measurements)
     size_t cl_smem = 0;
 };
-static std::vector<std::pair<const vc_circuit *, FusedHost>> g_fused;
+static std::vector<std::pair<const vc_circuit *, FusedHost *>> g_fused;   // heap entries: pointers handed out by find() stay valid
+static void release(FusedHost *f) {
+    if (!f) return;
+    cudaFree(f->d_plan); cudaFree(f->d_cta); cudaFree(f->d_slots); cudaFree(f->d_stamps); cudaFree(f->d_C); cudaFree(f->d_Tg); cudaFree(f->d_evcnt); cudaFree(f->d_cl);
+    delete f;
+}
 
 static FusedHost *find(const vc_circuit *c) {
-    for (auto &p : g_fused) if (p.first == c) return &p.second;
+    std::lock_guard<std::mutex> lk(g_registry_mutex);
+    for (auto &p : g_fused) if (p.first == c) return p.second;
     return nullptr;
 }
 
@@ -380,9 +387,17 @@ static cudaError_t launch_cluster(const ClArgs &a, int csize, size_t smem, cudaS
     return cudaLaunchKernelEx(&cfg, k_cluster, a);
 }
 
+static int fused_init_impl(vc_circuit *c, FusedHost &fh);
 int fused_init(vc_circuit *c) {
     if (!c->coop_ok) return VC_OK;
-    FusedHost fh;
+    FusedHost *fh = new (std::nothrow) FusedHost();
+    if (!fh) return VC_ERR_NOMEM;
+    const int rc = fused_init_impl(c, *fh);
+    if (rc != VC_OK || fh->grid == 0) { release(fh); return rc; }     // every partial allocation is returned; grid == 0: no fused schedule on this device
+    std::lock_guard<std::mutex> lk(g_registry_mutex);
+    return VC_OK;
+}
+static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
     fh.grid = c->sm_count;
     std::vector<LayerPlan> h(c->d + 1);
     std::vector<CtaPlan> all_cta;
@@ -410,11 +425,13 @@ int fused_init(vc_circuit *c) {
         cudaFuncSetAttribute(k_fused<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess ||
         cudaFuncSetAttribute(k_fused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) != cudaSuccess) {
         (void)cudaGetLastError();
+        fh.grid = 0;
         return VC_OK;                                // no fused schedule on this device; streaming still works
     }
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fused<7>, FT, fh.smem) != cudaSuccess || per_sm < 1) {
         (void)cudaGetLastError();
+        fh.grid = 0;
         return VC_OK;
     }
     uint64_t max_gates = 1;
@@ -442,14 +459,14 @@ int fused_init(vc_circuit *c) {
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     fh.group.resize(c->d);
     for (uint32_t i = 0; i < c->d; i++) fh.group[i] = h[i].kind == 0 ? 1 : (h[i].thin ? 2 : 4);
-    if (const char *e = getenv("VC_SINGLE_KERNEL")) g_single_kernel = e[0] == '1';
+    if (const char *e = getenv("VC_SINGLE_KERNEL")) fh.single_kernel = e[0] == '1';
     {   // the cluster engine takes every layer it can plan (VC_NO_CLUSTER=1: never, for A/B measurements)
         const char *nc = getenv("VC_NO_CLUSTER");
         std::vector<ClLayer> hc(c->d);
         size_t dyn = 0;
         const size_t fixed = (sizeof(ClShared) + 15) & ~(size_t)15;
         int csize = 0;
-        if (!(nc && nc[0] == '1') && !g_single_kernel &&
+        if (!(nc && nc[0] == '1') && !fh.single_kernel &&
             cudaFuncSetAttribute(k_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
             cudaFuncSetAttribute(k_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM_MAX) == cudaSuccess) {
             for (int cs : {CL_C, CL_C / 2}) {
@@ -484,15 +501,14 @@ int fused_init(vc_circuit *c) {
     if (!all_cta.empty() &&
         cudaMemcpy(fh.d_cta, all_cta.data(), all_cta.size() * sizeof(CtaPlan), cudaMemcpyHostToDevice) != cudaSuccess) return VC_ERR_CUDA;
     if (cudaMemset(fh.d_slots, 0, (size_t)F_RING * F_SLOT_WORDS * 8) != cudaSuccess) return VC_ERR_CUDA;
-    g_fused.emplace_back(c, fh);
     return VC_OK;
 }
 
 void fused_free(const vc_circuit *c) {
+    std::lock_guard<std::mutex> lk(g_registry_mutex);
     for (size_t i = 0; i < g_fused.size(); i++)
         if (g_fused[i].first == c) {
-            FusedHost &f = g_fused[i].second;
-            cudaFree(f.d_plan); cudaFree(f.d_cta); cudaFree(f.d_slots); cudaFree(f.d_stamps); cudaFree(f.d_C); cudaFree(f.d_Tg); cudaFree(f.d_evcnt); cudaFree(f.d_cl);
+            release(g_fused[i].second);
             g_fused.erase(g_fused.begin() + i);
             return;
         }
@@ -510,11 +526,15 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         const int m = fh->group[i];
         if (runs.empty() || runs.back().second != m || (m == 8 && i - runs.back().first >= CL_MAX_LAYERS)) runs.emplace_back(i, m);
     }
-    if (runs.size() > F_MAX_RUNS || g_single_kernel) {   // the all-kinds kernel cannot hold cluster layers: they keep their own launches
+    if (runs.size() > F_MAX_RUNS || fh->single_kernel) {   // the all-kinds kernel cannot hold cluster layers: they keep their own launches
         bool has_cl = false;
         for (auto &r : runs) has_cl = has_cl || r.second == 8;
         if (!has_cl) { runs.clear(); runs.emplace_back(begin, 7); }
         else for (auto &r : runs) if (r.second != 8) r.second = 7;
+    }
+    if (begin == 0) {   // a proof starts: the rendezvous slots and their epoch start clean whatever an earlier, aborted launch left behind
+        if (cudaMemsetAsync(fh->d_slots, 0, (size_t)F_RING * F_SLOT_WORDS * 8, st) != cudaSuccess ||
+            cudaMemsetAsync(&c->d_state->bar_gen, 0, sizeof(unsigned int), st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
     }
     uint64_t off = 0;
     for (size_t r = 0; r < runs.size(); r++) {

@@ -13,6 +13,7 @@
 // over the 7s+1 transcript words per layer, exactly as in vc_verify.cu, with the device sums plugged in.
 // Nothing here is shared with oracle/, nor with the prover's kernels beyond fp61.cuh.
 #include <algorithm>
+#include <new>
 #include <cstring>
 #include <vector>
 
@@ -177,10 +178,11 @@ struct VerifierHost {                                      // per circuit, alloc
     uint64_t *h_pin = nullptr;                             // transcript + results staging
     int blocks = 0;
 };
-static std::vector<std::pair<const vc_circuit *, VerifierHost>> g_verifiers;
+static std::vector<std::pair<const vc_circuit *, VerifierHost *>> g_verifiers;   // heap entries, guarded by g_registry_mutex
 
 static VerifierHost *verifier_of(const vc_circuit *c) {
-    for (auto &p : g_verifiers) if (p.first == c) return &p.second;
+    std::lock_guard<std::mutex> lk(g_registry_mutex);
+    for (auto &p : g_verifiers) if (p.first == c) return p.second;
     VerifierHost v;
     v.blocks = std::min(V_MAX_BLOCKS, 2 * c->sm_count);
     const size_t npts = (size_t)(c->d + 2) * 3 * MAX_VARS, nres = 4 * (size_t)c->d + 2;
@@ -194,15 +196,19 @@ static VerifierHost *verifier_of(const vc_circuit *c) {
     }
     cudaFuncSetAttribute(k_v_mle, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(V_TAB_WORDS * 8));
     cudaFuncSetAttribute(k_v_wiring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * V_TAB_WORDS * 8));
-    g_verifiers.emplace_back(c, v);
-    return &g_verifiers.back().second;
+    VerifierHost *hv = new (std::nothrow) VerifierHost(v);
+    if (!hv) { cudaFree(v.d_pts); cudaFree(v.d_res); cudaFree(v.d_part); cudaFree(v.d_flags); cudaFreeHost(v.h_pin); return nullptr; }
+    g_verifiers.emplace_back(c, hv);
+    return hv;
 }
 
 void verifier_free(const vc_circuit *c) {
+    std::lock_guard<std::mutex> lk(g_registry_mutex);
     for (size_t i = 0; i < g_verifiers.size(); i++)
         if (g_verifiers[i].first == c) {
-            VerifierHost &v = g_verifiers[i].second;
+            VerifierHost &v = *g_verifiers[i].second;
             cudaFree(v.d_pts); cudaFree(v.d_res); cudaFree(v.d_part); cudaFree(v.d_flags); cudaFreeHost(v.h_pin);
+            delete g_verifiers[i].second;
             g_verifiers.erase(g_verifiers.begin() + i);
             return;
         }
@@ -321,7 +327,8 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
  * type t of layer i, [1 + 4 d] the closing input extension */
 extern "C" int vc_debug_verifier_sums(const vc_circuit *c, uint64_t *h_sums, uint64_t n) {
     if (!c || !h_sums || n != 4 * (uint64_t)c->d + 2) return VC_ERR_ARG;
+    std::lock_guard<std::mutex> lk(vc::g_registry_mutex);
     for (auto &p : vc::g_verifiers)
-        if (p.first == c) { std::memcpy(h_sums, p.second.h_pin + c->total_words, n * 8); return VC_OK; }
+        if (p.first == c) { std::memcpy(h_sums, p.second->h_pin + c->total_words, n * 8); return VC_OK; }
     return VC_ERR_STATE;
 }

@@ -259,6 +259,64 @@ def test_non_canonical_input_is_flagged(vc):
     gc.close()
 
 
+def test_non_canonical_input_through_run_host_and_flag_is_per_evaluation(vc):
+    """include/vc.h (vc_evaluate, vc_run_host; SURVEY.md §8(b) "Errors"): a word >= p is detected on the device, reported by
+    vc_run_host as VC_ERR_ARG, and the status bit describes the LAST evaluation only: a valid input afterwards runs clean."""
+    import torch
+    c = W.random_circuit([2, 3, 5], 4, 8)
+    seed = 99
+    want_out, want_tr, _, _ = oracle.OracleCircuit(c).prove(c.input, seed)
+    gc = vc.Circuit(c)
+    bad = c.input.copy(); bad[3] = np.uint64(P + 5)
+    h_out = torch.zeros(gc.n_out, dtype=torch.int64).pin_memory()
+    h_tr = torch.zeros(gc.words, dtype=torch.int64).pin_memory()
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_run_host(gc.handle, torch.from_numpy(bad.view(np.int64)).pin_memory(), seed, h_out, h_tr)
+    assert e.value.code == vc.VC_ERR_ARG
+    assert gc.flags() & 1
+    vc.vc_run_host(gc.handle, torch.from_numpy(c.input.view(np.int64)).pin_memory(), seed, h_out, h_tr)   # same handle, valid input
+    assert gc.flags() == 0
+    assert np.array_equal(h_out.numpy().view(np.uint64), want_out) and np.array_equal(h_tr.numpy().view(np.uint64), want_tr)
+    gc.close()
+
+
+# ------------------------------------------------------------------ the cluster engine (layers of at most 2^12 gates)
+CLUSTER_CASES = [
+    ([10, 11, 12, 11, 10], 11, 41),     # 1 -> 8 -> 16 -> 8 -> 1... active CTAs grow and shrink: state hand-over to CTAs that join
+    ([12, 4, 12, 3], 9, 42),            # a wide cluster layer after a single-CTA one, twice; tables of 2^4 .. 2^12 words
+    ([11, 14, 9], 12, 43),              # irregular wiring into a 2^14 table: every CTA holds the whole table (no slices)
+    ([0, 12], 12, 44),                  # one output reading a 2^12 layer: start claim on one gate, line restriction in blocks
+]
+
+
+@pytest.mark.parametrize("log_sizes,log_input,seed", CLUSTER_CASES)
+def test_cluster_engine_random_circuits_bit_exact(vc, log_sizes, log_input, seed):
+    c = W.random_circuit(log_sizes, log_input, seed)
+    want_out, want_tr, want_z, want_claim = oracle.OracleCircuit(c).prove(c.input, 900 + seed)
+    for layerwise in (False, True):      # one launch for the run of layers, or one launch per layer (state through DevState)
+        gc, out, tr = _gpu_prove(vc, c, 900 + seed, 0, layerwise=layerwise)
+        assert np.array_equal(out, want_out)
+        bad = np.nonzero(tr != want_tr)[0]
+        assert bad.size == 0, f"layerwise={layerwise}: first mismatch at word {bad[:5]} of {tr.size}"
+        z, claim, _ = gc.state()
+        assert claim == want_claim and np.array_equal(z[:c.log_input], want_z[:c.log_input])
+        gc.close()
+
+
+def test_cluster_engine_and_grid_kernels_give_the_same_transcript(vc, monkeypatch):
+    """VC_NO_CLUSTER=1 at load keeps every layer on the grid-wide kernels: both routes must give the oracle's words (the
+    structured circuits put tree, self and two-lane chain wiring through the cluster engine's sliced tables)."""
+    for c, seed in [(W.f0_circuit(9, 5), 51), (W.matmul_circuit(4, 6), 52), (W.pm_circuit(9, 3, 7, planted=3), 53)]:
+        want_out, want_tr, _, want_claim = oracle.OracleCircuit(c).prove(c.input, seed)
+        for off in ("0", "1"):
+            monkeypatch.setenv("VC_NO_CLUSTER", off)
+            gc, out, tr = _gpu_prove(vc, c, seed)
+            assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (c.name, off)
+            assert gc.state()[1] == want_claim
+            gc.close()
+    monkeypatch.delenv("VC_NO_CLUSTER")
+
+
 def test_run_host_end_to_end_matches(vc):
     import torch
     c = W.config(1)

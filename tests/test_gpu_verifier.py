@@ -140,11 +140,55 @@ def test_device_verifier_on_configs(vc, k):
     gc.close()
 
 
+def _check_against_paper_golden(kind, n, c, out, tr, claim):
+    """Word-for-word parity with the oracle at a paper-scale size: tests/golden/paper_<kind>_<n>.txt holds the per-layer
+    SHA-256 digests of the ORACLE's transcript (tests/golden/make_golden.py <kind>:<n>, oracle/ only), same seeds as here."""
+    import hashlib
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"paper_{kind}_{n}.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated (python tests/golden/make_golden.py {kind}:{n})")
+    sha = lambda a: hashlib.sha256(np.ascontiguousarray(a, dtype="<u8").tobytes()).hexdigest()
+    g, layers = {}, {}
+    for line in open(path):
+        if line.startswith("#"):
+            continue
+        p_ = line.split()
+        if p_[0] == "layer":
+            layers[int(p_[1])] = (p_[3], int(p_[4]), int(p_[5]))
+        else:
+            g[p_[0]] = p_[1]
+    assert int(g["gates"]) == c.gates and int(g["transcript_words"]) == tr.size
+    assert sha(out) == g["outputs_sha256"] and int(out[0]) == int(g["output0"])
+    w = 0
+    for i in range(c.d):
+        nw = c.transcript_words(i)
+        seg = tr[w:w + nw]
+        digest, first, last = layers[i]
+        assert (int(seg[0]), int(seg[-1])) == (first, last), f"{kind}:{n} layer {i}"
+        assert sha(seg) == digest, f"{kind}:{n} layer {i}"
+        w += nw
+    assert sha(tr) == g["transcript_sha256"] and claim == int(g["final_claim"])
+
+
+def test_f2_2_22_tree_layers_on_global_state_match_the_oracle(vc):
+    """F2 at n = 2^22: its 2^21-gate ADD-tree layer is the implicit-TREE wiring with NON-resident gate state (global scratch),
+    a kernel branch no BASELINE.json config reaches.  Oracle digests: tests/golden/paper_f2_22.txt."""
+    from vc_workloads import circuits
+    c = circuits.f2_circuit(22, 7)
+    gc = vc.Circuit(c)
+    gc.set_input(c.input)
+    gc.evaluate(); gc.prove(31337)
+    assert gc.flags() == 0
+    _check_against_paper_golden("f2", 22, c, gc.outputs().copy(), gc.transcript().copy(), gc.state()[1])
+    gc.close()
+
+
 def test_paper_scale_f2_runs_and_verifies(vc):
     """the F2 construction at the paper's largest size, n = 2^23 (25.2 M nodes with the inputs,
-    Table 2).  Too large for the oracle in a test, so properties that hold at any size: the output is the
-    directly computed sum of squares, the device verifier accepts the transcript and rejects flipped words, the host
-    verifier of the library agrees on a sample."""
+    Table 2).  The transcript is compared layer by layer with the oracle's digests
+    (tests/golden/paper_f2_23.txt, written by the oracle alone in ~2 min); on top of that properties that hold at any
+    size: the output is the directly computed sum of squares, the device verifier accepts and rejects flipped words."""
     from vc_workloads import circuits
     c = circuits.f2_circuit(23, 7)
     gc = vc.Circuit(c)
@@ -153,6 +197,7 @@ def test_paper_scale_f2_runs_and_verifies(vc):
     assert gc.flags() == 0
     out, tr = gc.outputs().copy(), gc.transcript().copy()
     assert int(out[0]) == int((c.input.astype(np.uint64) ** 2).sum(dtype=np.uint64)) % P     # < 2^63: no wrap
+    _check_against_paper_golden("f2", 23, c, out, tr, gc.state()[1])                          # the oracle's transcript, layer by layer
     assert gc.verify_device(31337) == (True, 0, 0)
     # round invariant on the whole transcript's first layer and a late one (g(0) + g(1) = claim chain is what V checks)
     rng = np.random.default_rng(5)
@@ -168,8 +213,10 @@ def test_paper_scale_f2_runs_and_verifies(vc):
 @pytest.mark.parametrize("kind,n", [("matmul", 8), ("pm", 19), ("f0", 20)])
 def test_paper_scale_other_constructions(vc, kind, n):
     """MATMULT 256 x 256, PM with 2^19 text symbols (Table 2's sizes) and F0 at
-    2^20 (half of Table 2's 2^21: the host arrays of 2^21 double the test's memory for no new code path).  Properties that
-    hold at any size: outputs equal the directly computed values, the device verifier accepts, a flipped word is rejected."""
+    2^20 (half of Table 2's 2^21: the oracle needs ~20 min and 9 GB for 2^21, and no new code path is reached; bench.py
+    --paper-scale f0:21 times it).  Transcripts are compared with the oracle's per-layer digests
+    (tests/golden/paper_<kind>_<n>.txt); also: outputs equal the directly computed values, the device verifier accepts,
+    a flipped word is rejected."""
     from vc_workloads import circuits
     c = {"matmul": lambda: circuits.matmul_circuit(n, 4), "pm": lambda: circuits.pm_circuit(n, 3, 5),
          "f0": lambda: circuits.f0_circuit(n, 3)}[kind]()
@@ -187,6 +234,7 @@ def test_paper_scale_other_constructions(vc, kind, n):
         assert int(out[0]) == int(T - match.sum())                                              # reading c-13: non-matching cyclic offsets
     else:
         assert int(out[0]) == int(np.count_nonzero(c.input))
+    _check_against_paper_golden(kind, n, c, out, tr, gc.state()[1])   # the oracle's transcript, layer by layer (skips if the digest file is absent)
     assert gc.verify_device(4242) == (True, 0, 0)
     rng = np.random.default_rng(n)
     for w in rng.integers(0, tr.size, size=2):
