@@ -52,10 +52,10 @@ def algorithmic_counts(c):
         mm_eval = int(np.count_nonzero(L.type == W.MULT))
         per_layer.append(dict(n=n, s=s, prove_bytes=rounds_bytes + table_bytes + line_bytes + beta_bytes,
                               round_bytes=[n * (17 + (8 if ph == 1 else 0)) + 8 * (nb >> j) for ph in (1, 2) for j in range(s)],
-                              eval_bytes=eval_bytes, modmul=mm + mm_eval))
+                              eval_bytes=eval_bytes, modmul=mm, modmul_eval=mm_eval))
     return dict(layers=per_layer,
                 bytes=sum(l["prove_bytes"] + l["eval_bytes"] for l in per_layer),
-                modmul=sum(l["modmul"] for l in per_layer))
+                modmul=sum(l["modmul"] + l["modmul_eval"] for l in per_layer))
 
 
 def measured_peaks():
@@ -119,8 +119,23 @@ def oracle_sample_step(oc, c, V, seed, layers):
     return gr
 
 
+def workload_config(c, k, world=1, schedule=0):
+    """The `config` object of the bench line: the same keys for both arms."""
+    return {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}" if k else f"paper scale (not a BASELINE.json config): {c.name}",
+            "gates": c.gates, "layers": c.d, "rounds": c.rounds, "gate_rounds": c.gate_rounds, "replicas": world,
+            "schedule": schedule}
+
+
 def run_reference(args):
-    """--impl reference: the CPU oracle on the host cores (rank 0 only), bounded sample per step."""
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only).
+
+    There is no reference implementation to install (/root/reference holds PAPER.md only), so the reference arm is the
+    oracle.  One whole oracle proof of config 2 takes ~6 s: a step is therefore a BOUNDED SAMPLE of the workload — evaluate
+    the circuit, then prove a fixed set of its layers in isolation (their entry state comes from the counter-based
+    draws) — and `value` is the throughput of that sample in the metric's unit: the sample's share of the circuit's gates
+    (by gate-rounds, the oracle's cost driver) divided by the measured time of the step.  `ms_per_step` is the measured
+    time of the sample, nothing is extrapolated.
+    """
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -129,7 +144,7 @@ def run_reference(args):
     c = W.config(k)
     seed = W.challenge_seed(k)
     oc = oracle.OracleCircuit(c)
-    # sample: the layers whose gate-rounds sum to ~5 M (about a second of oracle time), widest first that fits
+    # sample: the layers whose gate-rounds sum to ~6 M (about half a second of oracle time), widest first that fits
     order = sorted(range(c.d), key=lambda i: -(1 << c.layers[i].log_size) * c.log_below(i))
     budget, layers, tot = 6_000_000, [], 0
     for i in order:
@@ -146,16 +161,17 @@ def run_reference(args):
     for _ in range(args.steps):
         V = oc.evaluate(c.input)
         gr += oracle_sample_step(oc, c, V, seed, layers)
-    dt = (time.perf_counter() - t0) / args.steps
+    dt = (time.perf_counter() - t0) / args.steps          # measured seconds per step (one sample)
     gr //= args.steps
-    full = dt * c.gate_rounds / gr                       # oracle time is ~proportional to gate-rounds
-    value = c.gates / full
+    sample_gates = c.gates * gr / c.gate_rounds            # the sample's share of the circuit, in gates
+    value = sample_gates / dt
     sample = (f"per step: evaluate + oracle proof of layers {layers[0]}..{layers[-1]} ({len(layers)} layers, {gr} of "
-              f"{c.gate_rounds} gate-rounds) in isolation; whole-proof time extrapolated by gate-rounds")
+              f"{c.gate_rounds} gate-rounds = {sample_gates:.0f} gate-equivalents) in isolation, {dt:.3f} s measured; "
+              f"value = gate-equivalents / measured time, no extrapolation")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}" if k else f"paper scale (not a BASELINE.json config): {c.name}", "gates": c.gates},
+            "config": workload_config(c, k, 1, 0),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -265,55 +281,84 @@ def run_ours(args):
     e2e_value = replicas.whole_job_value(c.gates, world, e2e_ms / args.steps)
 
     if rank == 0:
-        # ---- per-kernel-kind timing (CUDA events inside the library, on the launching stream), one extra step
+        # ---- per-kernel-kind timing (CUDA events inside the library, on the launching stream), three extra steps
         counts = algorithmic_counts(c)
         peak, peak_src = measured_peaks()
-        L.vc_profile_enable(1)
-        flush.fill_(1)
-        step()
         nk = 10
-        pl, pm = (C.c_uint64 * nk)(), (C.c_double * nk)()
-        L.vc_profile_read(pl, pm)
-        L.vc_profile_enable(0)
         kinds = ["evaluate", "setup(beta,start)", "round", "update+fold", "line", "fused_narrow", "fused_wide", "misc", "fused_thin", "cluster"]
-        prof = {kinds[i]: {"launches": int(pl[i]), "ms": round(float(pm[i]), 4)} for i in range(nk) if pl[i]}
+        acc_l, acc_ms, nprof = [0] * nk, [0.0] * nk, 3
+        for _ in range(nprof):
+            flush.fill_(1)
+            L.vc_profile_enable(1)
+            step()
+            pl, pm = (C.c_uint64 * nk)(), (C.c_double * nk)()
+            L.vc_profile_read(pl, pm)
+            L.vc_profile_enable(0)
+            for i in range(nk):
+                acc_l[i] += int(pl[i]); acc_ms[i] += float(pm[i])
+        prof = {kinds[i]: {"launches": acc_l[i] // nprof, "ms": round(acc_ms[i] / nprof, 4)} for i in range(nk) if acc_l[i]}
         prof_total = sum(v["ms"] for v in prof.values())
-        dom = max(prof, key=lambda n: prof[n]["ms"])
-        if dom == "round":
-            dom_bytes = sum(sum(l["round_bytes"]) for l in counts["layers"])
-            dom_desc = "k_round<phase>: per launch n*(9 B record + 8 B weight [+ 8 B operand in phase 1]) + 8*2^(s-j) B table"
-        else:
-            dom_bytes = counts["bytes"] * (prof[dom]["ms"] / prof_total)
-            dom_desc = f"{dom}: share of the step's algorithmic bytes by time"
-        ach = dom_bytes / (prof[dom]["ms"] * 1e-3) / 1e9
-        # integer-multiply rate (fp61 multiplies/s) measured live: 8 independent chains per thread
-        outw = torch.empty(148 * 8 * 256, dtype=torch.int64, device="cuda")
+        # algorithmic bytes / multiplies of every kernel kind: the layers IT proves (the library says which), its own time
+        kind_bytes, kind_mm = {kk: 0 for kk in kinds}, {kk: 0 for kk in kinds}
+        try:
+            lk = gc.layer_kinds() if args.schedule == 0 else None
+        except Exception:
+            lk = None
+        for i, lay in enumerate(counts["layers"]):
+            kind_bytes["evaluate"] += lay["eval_bytes"]; kind_mm["evaluate"] += lay["modmul_eval"]
+            if lk is not None:
+                kind_bytes[kinds[int(lk[i])]] += lay["prove_bytes"]; kind_mm[kinds[int(lk[i])]] += lay["modmul"]
+            else:                                # streaming schedule: split by step as algorithmic_counts does
+                kind_bytes["round"] += sum(lay["round_bytes"]); kind_mm["round"] += 2 * lay["n"] * 2 * lay["s"]
+        # integer-multiply rate (fp61 multiplies/s) measured live: 8 independent chains per thread, one CTA set per SM
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        outw = torch.empty(sms * 8 * 256, dtype=torch.int64, device="cuda")
         best = 0.0
         for _ in range(3):
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
-            L.vc_bench_modmul(148 * 8, 256, 4096, 8, outw.data_ptr(), stream.cuda_stream)
+            L.vc_bench_modmul(sms * 8, 256, 4096, 8, outw.data_ptr(), stream.cuda_stream)
             b.record(stream)
             torch.cuda.synchronize()
-            best = max(best, 148 * 8 * 256 * 4096 * 8 / (a.elapsed_time(b) * 1e-3))
+            best = max(best, sms * 8 * 256 * 4096 * 8 / (a.elapsed_time(b) * 1e-3))
+        for kk, v in prof.items():
+            if kind_bytes.get(kk):
+                v["algorithmic_bytes"] = int(kind_bytes[kk]); v["algorithmic_modmul"] = int(kind_mm[kk])
+                v["algorithmic_GBps"] = round(kind_bytes[kk] / (v["ms"] * 1e-3) / 1e9, 1)
+                v["hbm_frac"] = round(kind_bytes[kk] / (peak * 1e9) / (v["ms"] * 1e-3), 4)
+                v["alu_frac"] = round(kind_mm[kk] / best / (v["ms"] * 1e-3), 4)
+        dom = max(prof, key=lambda n_: prof[n_]["ms"])
+        dom_bytes, dom_mm, dom_ms = kind_bytes.get(dom, 0), kind_mm.get(dom, 0), prof[dom]["ms"]
+        ach = dom_bytes / (dom_ms * 1e-3) / 1e9
         t_hbm = counts["bytes"] / (peak * 1e9)
         t_alu = counts["modmul"] / best
         roof_ms = max(t_hbm, t_alu) * 1e3
-        traffic = None                           # dram bytes of the dominant kernel, from the committed ncu capture
+        # which bound is the slower one FOR THE DOMINANT KERNEL (BASELINE.json north_star: the roofline is the slower of the two)
+        dom_hbm_ms, dom_alu_ms = dom_bytes / (peak * 1e9) * 1e3, dom_mm / best * 1e3
+        traffic, traffic_src = None, None         # DRAM bytes of the dominant kernel from the committed ncu capture (not measured in this run)
         try:
-            with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
                 tj = json.load(f)
-            if k == 2 and args.schedule == 0 and dom == "fused_wide":
+            if k == 2 and args.schedule == 0 and tj.get("kernel_kind") == dom:
                 traffic = int(tj["dram_bytes_read"]) + int(tj["dram_bytes_write"])
+                traffic_src = f"profiles/r02_traffic.json (ncu --set full capture of commit {tj.get('commit', '?')}, one launch)"
         except Exception:
             pass
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": traffic, "peak_source": peak_src, "what": dom_desc,
-                    "kernel_share_of_step": prof[dom]["ms"] / prof_total, "per_kind": prof,
+        roofline = {"bound": "hbm" if dom_hbm_ms >= dom_alu_ms else "alu", "kernel": dom,
+                    "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                    "what": (f"{dom}: ALGORITHMIC bytes of the layers this kernel proves (SURVEY.md §8(d): 33/25 B per gate-round + tables + "
+                             f"line pass + beta write) / its own CUDA-event time, averaged over {nprof} launches; not DRAM traffic "
+                             f"(the working set is shared-memory/L2 resident: see `traffic`)"),
+                    "kernel_ms": dom_ms, "kernel_algorithmic_bytes": int(dom_bytes), "kernel_algorithmic_modmul": int(dom_mm),
+                    "kernel_hbm_bound_ms": dom_hbm_ms, "kernel_alu_bound_ms": dom_alu_ms,
+                    "frac_at_8TBps": dom_bytes / 8e12 * 1e3 / dom_ms, "alu_frac": dom_alu_ms / dom_ms,
+                    "kernel_share_of_step": dom_ms / prof_total, "per_kind": prof,
                     "step": {"algorithmic_bytes": counts["bytes"], "algorithmic_modmul": counts["modmul"],
                              "hbm_bound_ms": t_hbm * 1e3, "modmul_rate_per_s": best, "alu_bound_ms": t_alu * 1e3,
                              "roofline_ms": roof_ms, "frac": roof_ms / ms_per_step,
-                             "frac_at_8TBps": counts["bytes"] / 8e12 * 1e3 / ms_per_step}}
+                             "frac_at_8TBps": counts["bytes"] / 8e12 * 1e3 / ms_per_step,
+                             "alu_frac": t_alu * 1e3 / ms_per_step}}
         # ---- NEXT-1: the verifier with its O(S) sums on the GPU, beside the library's host verifier
         # (outside the timed region; wall clock around the synchronous calls)
         verifier = None
@@ -352,10 +397,9 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "u64 (F_p, p=2^61-1)", "data": "synthetic",
-                "config": {"workload": f"BASELINE.json configs[{k - 1}]: {c.name}" if k else f"paper scale (not a BASELINE.json config): {c.name}", "gates": c.gates, "layers": c.d,
-                           "rounds": c.rounds, "gate_rounds": c.gate_rounds, "replicas": world,
-                           "schedule": args.schedule, "l2": "flushed between steps (256 MiB fill, outside the event pairs)",
-                           "ms_min": min(ms), "ms_median": float(np.median(ms))},
+                "config": dict(workload_config(c, k, world, args.schedule),
+                               l2="flushed between steps (256 MiB fill, outside the event pairs)",
+                               ms_min=min(ms), ms_median=float(np.median(ms))),
                 "clocks": clocks, "gpu_launches": launches,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(c.input.nbytes),
                         "d2h_bytes_per_step": int(8 * (gc.n_out + gc.words)), "ms_per_step": e2e_ms / args.steps},

@@ -124,6 +124,10 @@ int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, voi
 int vc_debug_verifier_sums(const vc_circuit *c, uint64_t *h_sums, uint64_t n);
 /* device-side status of the last vc_evaluate on this handle: 0 = fine, bit 0 = a non-canonical input word was seen */
 int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
+/* which kernel proves each layer on the fused schedule: h_kind receives d words, each one of VC_K_CLUSTER, VC_K_FUSED_NARROW,
+ * VC_K_FUSED_THIN, VC_K_FUSED_WIDE (bench.py uses it to give every kernel kind its own algorithmic byte count);
+ * VC_ERR_STATE when the circuit has no fused plan (streaming schedule only) */
+int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */
 uint64_t vc_launch_count(void);
 /* selects the kernel schedule: 0 = auto (default), see DESIGN.md "Schedules" for the others */

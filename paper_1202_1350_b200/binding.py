@@ -16,7 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
-    "vc_verify_transcript_device", "vc_debug_verifier_sums",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds",
 ]
 
 
@@ -70,6 +70,7 @@ def lib():
             "vc_bench_modmul": (i32, [u32, u32, u32, u32, vp, vp]),
             "vc_debug_layer_stamps": (i32, [vp, vp, vp]),
             "vc_debug_trace": (i32, [vp, vp, u32, vp]),
+            "vc_debug_layer_kinds": (i32, [vp, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
         }
@@ -241,6 +242,12 @@ class Circuit:
         """d+1 device timestamps (ns) of the last fused proof: start of each layer, [d] = end (vc_debug_layer_stamps)."""
         h = np.zeros(self.d + 1, dtype=np.uint64)
         _check(lib().vc_debug_layer_stamps(self.handle, _host_ptr(h), None), "vc_debug_layer_stamps")
+        return h
+
+    def layer_kinds(self) -> np.ndarray:
+        """Per layer, the VC_K_* code of the kernel that proves it on the fused schedule (vc_debug_layer_kinds)."""
+        h = np.zeros(self.d, dtype=np.uint32)
+        _check(lib().vc_debug_layer_kinds(self.handle, h.ctypes.data), "vc_debug_layer_kinds")
         return h
 
     def flags(self) -> int:

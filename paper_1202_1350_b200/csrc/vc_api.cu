@@ -305,6 +305,11 @@ extern "C" int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *
     return vc::fused_stamps(c, h_ns, (cudaStream_t)cuda_stream);
 }
 
+extern "C" int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind) {
+    if (!c || !h_kind) return VC_ERR_ARG;
+    return vc::fused_layer_kinds(c, h_kind);
+}
+
 extern "C" int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, void *cuda_stream) {
     if (!c || !h_words) return VC_ERR_ARG;
     return vc::fused_trace(c, h_words, n_words, (cudaStream_t)cuda_stream);

@@ -54,6 +54,7 @@ int fused_init(vc_circuit *c);
 void fused_free(const vc_circuit *c);
 void verifier_free(const vc_circuit *c);   // vc_verify_gpu.cu
 int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st);
+int fused_layer_kinds(const vc_circuit *c, uint32_t *h_kind);
 int fused_trace(const vc_circuit *c, uint64_t *h, uint32_t n_words, cudaStream_t st);
 int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, cudaStream_t st);
 int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t seed, uint64_t *d_tr, cudaStream_t st);

@@ -395,6 +395,7 @@ int fused_init(vc_circuit *c) {
     const int rc = fused_init_impl(c, *fh);
     if (rc != VC_OK || fh->grid == 0) { release(fh); return rc; }     // every partial allocation is returned; grid == 0: no fused schedule on this device
     std::lock_guard<std::mutex> lk(g_registry_mutex);
+    g_fused.emplace_back(c, fh);
     return VC_OK;
 }
 static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
@@ -563,6 +564,16 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
         for (uint32_t i = b0; i < e0; i++) off += 7ull * c->logs[i + 1] + 1;
+    }
+    return VC_OK;
+}
+
+int fused_layer_kinds(const vc_circuit *c, uint32_t *h_kind) {
+    FusedHost *fh = find(c);
+    if (!fh) return VC_ERR_STATE;
+    for (uint32_t i = 0; i < c->d; i++) {
+        const int g = fh->group[i];
+        h_kind[i] = g == 8 ? VC_K_CLUSTER : g == 1 ? VC_K_FUSED_NARROW : g == 2 ? VC_K_FUSED_THIN : VC_K_FUSED_WIDE;
     }
     return VC_OK;
 }

@@ -280,6 +280,23 @@ def test_non_canonical_input_through_run_host_and_flag_is_per_evaluation(vc):
     gc.close()
 
 
+def test_default_schedule_is_the_fused_one_not_a_silent_fallback(vc):
+    """The streaming schedule is always available and gives the same words, so a broken fused plan would pass every parity
+    test unnoticed: check that schedule 0 really runs the persistent kernels (a handful of launches per proof, a kernel kind
+    for every layer) and that config 2's layers go where the plan says (cluster engine up to 2^12 gates, grid above)."""
+    c = W.config(2)
+    gc = vc.Circuit(c)
+    kinds = gc.layer_kinds()                      # raises VC_ERR_STATE if the circuit has no fused plan
+    K = vc.lib()
+    assert list(kinds[:13]) == [9] * 13           # VC_K_CLUSTER
+    assert set(int(x) for x in kinds[13:]) <= {6, 8}   # VC_K_FUSED_WIDE / VC_K_FUSED_THIN
+    gc.set_input(c.input)
+    n0 = K.vc_launch_count()
+    gc.evaluate(); gc.prove(W.challenge_seed(2))
+    assert K.vc_launch_count() - n0 <= 6          # evaluation + one launch per run of layer kinds
+    gc.close()
+
+
 # ------------------------------------------------------------------ the cluster engine (layers of at most 2^12 gates)
 CLUSTER_CASES = [
     ([10, 11, 12, 11, 10], 11, 41),     # 1 -> 8 -> 16 -> 8 -> 1... active CTAs grow and shrink: state hand-over to CTAs that join
