@@ -1,5 +1,6 @@
 // vc_fused.cu — kernel + host driver (load-time plan, launch) of the on-chip schedule (see vc_fused.cuh).
 #include <algorithm>
+#include <cstdio>
 #include <new>
 #include <cstdlib>
 #include <vector>
@@ -241,6 +242,22 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
             nbmax[ph] = std::max<uint64_t>(nbmax[ph], cta[b].nb[ph]);
         }
     }
+    // level K-1 published from the slices: CTAs in order take the entries of their slice nobody before them took; that
+    // works when the slices cover the whole level without a gap (regular wiring), else the owners compute their entries from V
+    bool cover[2] = {K >= 2, K >= 2};
+    for (int ph = 0; ph < 2; ph++) {
+        const uint64_t E = 1ull << (s - K + 1);
+        uint64_t next = 0;
+        for (int b = 0; b < G && cover[ph]; b++) {
+            cta[b].own_lo[ph] = cta[b].own_n[ph] = 0;
+            if (cta[b].g1 == cta[b].g0) continue;
+            const uint64_t lo = 2ull * cta[b].blo[ph], hi = 2ull * ((uint64_t)cta[b].blo[ph] + cta[b].nb[ph]);
+            if (lo > next) { cover[ph] = false; break; }
+            if (hi > next) { cta[b].own_lo[ph] = (uint32_t)next; cta[b].own_n[ph] = (uint32_t)(hi - next); next = hi; }
+        }
+        if (next != E) cover[ph] = false;
+        if (getenv("VC_NO_PUB_SLICE")) cover[ph] = false;
+    }
     const size_t cap = (size_t)((ngmax + FT - 1) / FT) * FT;
     const size_t state = cap * 20;
     // fold buffers: odd levels in X, even levels in Y; slices exist for levels 1..K-1
@@ -264,7 +281,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         if (total <= F_SMEM_MAX) {
             lp.thin = ngmax <= F_WORKERS / 4 ? 4 : 1;        // lanes per gate
             lp.cap = (uint32_t)cap;
-            for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = F_MODE_SLICE; lp.K[ph] = K; }
+            for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = F_MODE_SLICE; lp.K[ph] = K; lp.pub_slice[ph] = cover[ph] ? 1u : 0u; }
             lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
             lp.off_tab = (uint32_t)F_THIN_COMMIT_BYTES;
             lp.off_scr = (uint32_t)(F_THIN_COMMIT_BYTES + tabw * 8);
@@ -292,7 +309,7 @@ static void plan_layer(const vc_circuit *c, uint32_t i, int G, LayerPlan &lp, st
         if (total > F_SMEM_MAX) continue;
         lp.resident = res ? 1 : 0;
         lp.cap = (uint32_t)cap;
-        for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = use[ph] ? F_MODE_SLICE : F_MODE_GLOBAL; lp.K[ph] = K; }
+        for (int ph = 0; ph < 2; ph++) { lp.mode[ph] = use[ph] ? F_MODE_SLICE : F_MODE_GLOBAL; lp.K[ph] = K; lp.pub_slice[ph] = (use[ph] && cover[ph]) ? 1u : 0u; }
         lp.xw = (uint32_t)X; lp.yw = (uint32_t)Y;
         lp.off_tab = (uint32_t)st_bytes;
         lp.off_scr = (uint32_t)(st_bytes + tabw * 8);

@@ -37,6 +37,7 @@ constexpr int F_MODE_SLICE = 0, F_MODE_GLOBAL = 1;
 struct CtaPlan {                         // per (wide layer, CTA), computed at load from the host copy of the records
     uint32_t g0, g1;                     // gates [g0, g1) of the layer
     uint32_t blo[2], nb[2];              // per phase: first level-K block its gates read, and how many
+    uint32_t own_lo[2], own_n[2];        // per phase (LayerPlan::pub_slice): the entries of level K-1 this CTA publishes from its own slice
 };
 
 struct LayerPlan {
@@ -53,6 +54,8 @@ struct LayerPlan {
     uint32_t cap;                        // state capacity in gates (multiple of FT)
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
+    uint32_t pub_slice[2];               // per phase: 1 = the CTAs' slices cover level K-1 of the whole table, so each CTA publishes the entries
+                                         // it owns straight from its slice (no pass over V_{i+1} with an eq table)
     uint32_t xw, yw;                     // words of the two fold buffers
     uint32_t off_tab, off_scr, off_commit;   // byte offsets in dynamic shared memory (after the state)
 };

@@ -98,8 +98,24 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
         for (uint32_t j = 0; j < s; j++) {
             bool fence = false;
             if (K >= 2 && j == K - 1) {              // publish level K-1 (read by round K's gates and by its level build)
-                const uint32_t E = 1u << (s - K + 1);
-                publish_level(Vb, rr, K - 1, (uint32_t)(((uint64_t)b * E) / G), (uint32_t)(((uint64_t)(b + 1) * E) / G), scr, a.Tg);
+                if (Lp.pub_slice[ph]) {              // the slices cover the level: fold this CTA's share from level K-2 of its slice
+                    __syncthreads();                 // level K-2 (built in the shadow of the last rendezvous) and r_prev are in place
+                    const uint32_t o0 = cp.own_lo[ph], on = cp.own_n[ph];
+                    for (uint32_t e = tid; e < on; e += FT) {
+                        const uint32_t idx = o0 + e;
+                        uint64_t x0, x1;
+                        if (K == 2) { const ulonglong2 p = __ldg(reinterpret_cast<const ulonglong2 *>(Vb + 2 * (size_t)idx)); x0 = p.x; x1 = p.y; }
+                        else {
+                            const uint64_t *src = ((K - 2) & 1) ? bufX : bufY;
+                            const ulonglong2 p = *reinterpret_cast<const ulonglong2 *>(src + (2 * (size_t)idx - ((size_t)blo << 2)));
+                            x0 = p.x; x1 = p.y;
+                        }
+                        __stcg(a.Tg + idx, fold2(x0, x1, r_prev));
+                    }
+                } else {
+                    const uint32_t E = 1u << (s - K + 1);
+                    publish_level(Vb, rr, K - 1, (uint32_t)(((uint64_t)b * E) / G), (uint32_t)(((uint64_t)(b + 1) * E) / G), scr, a.Tg);
+                }
                 fence = true;
             }
             // ---- a4 for this thread's gate, against level j-1 folded on the fly (level 0 in round 0)

@@ -356,8 +356,15 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                     tab = dst;
                 }
                 if (K >= 2 && j == K - 1) {      // publish level K-1 for the next round (needs r_0..r_{K-2})
-                    const uint32_t E = 1u << (s - K + 1);
-                    publish_level(Vb, rr, K - 1, (uint32_t)(((uint64_t)b * E) / G), (uint32_t)(((uint64_t)(b + 1) * E) / G), scr, a.Tg);
+                    if (Lp.pub_slice[ph]) {      // the slices cover the level: this CTA's share is in the slice it has just folded
+                        __syncthreads();
+                        const uint64_t *lvl = (j & 1) ? bufX : bufY;
+                        const uint32_t o0 = cp.own_lo[ph], on = cp.own_n[ph], sb0 = blo << 1;
+                        for (uint32_t e = tid; e < on; e += GT) __stcg(a.Tg + o0 + e, lvl[o0 + e - sb0]);
+                    } else {
+                        const uint32_t E = 1u << (s - K + 1);
+                        publish_level(Vb, rr, K - 1, (uint32_t)(((uint64_t)b * E) / G), (uint32_t)(((uint64_t)(b + 1) * E) / G), scr, a.Tg);
+                    }
                     fence = true;
                 }
             } else {                             // GLOBAL: materialise level j (j >= 1) for the next round's on-the-fly fold
