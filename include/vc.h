@@ -128,6 +128,11 @@ int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
  * VC_K_FUSED_THIN, VC_K_FUSED_WIDE (bench.py uses it to give every kernel kind its own algorithmic byte count);
  * VC_ERR_STATE when the circuit has no fused plan (streaming schedule only) */
 int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind);
+/* how the prover obtains each layer's wiring (the paper's §5.1.4 computes the tree's indices instead of
+ * loading them): h_mode receives d words, 0 = the stored records are read, 1 = binary tree (2g, 2g+1) computed, 2 = in1 = in2 = g
+ * computed, 3 = computed from the bit-field rule vc_load fitted to the records and checked against every one of them.  The
+ * records stay the definition: a layer gets a computed mode only when it reproduces all of its records. */
+int vc_debug_layer_wiring(const vc_circuit *c, uint32_t *h_mode);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */
 uint64_t vc_launch_count(void);
 /* selects the kernel schedule: 0 = auto (default), see DESIGN.md "Schedules" for the others */

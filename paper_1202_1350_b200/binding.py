@@ -16,7 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
-    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring",
 ]
 
 
@@ -71,6 +71,7 @@ def lib():
             "vc_debug_layer_stamps": (i32, [vp, vp, vp]),
             "vc_debug_trace": (i32, [vp, vp, u32, vp]),
             "vc_debug_layer_kinds": (i32, [vp, vp]),
+            "vc_debug_layer_wiring": (i32, [vp, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
         }
@@ -248,6 +249,12 @@ class Circuit:
         """Per layer, the VC_K_* code of the kernel that proves it on the fused schedule (vc_debug_layer_kinds)."""
         h = np.zeros(self.d, dtype=np.uint32)
         _check(lib().vc_debug_layer_kinds(self.handle, h.ctypes.data), "vc_debug_layer_kinds")
+        return h
+
+    def layer_wiring(self) -> np.ndarray:
+        """Per layer, how the prover gets its wiring: 0 records, 1 tree, 2 self, 3 bit-field rule (vc_debug_layer_wiring)."""
+        h = np.zeros(self.d, dtype=np.uint32)
+        _check(lib().vc_debug_layer_wiring(self.handle, h.ctypes.data), "vc_debug_layer_wiring")
         return h
 
     def flags(self) -> int:

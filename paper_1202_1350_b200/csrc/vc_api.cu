@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -67,6 +68,49 @@ extern "C" void vc_circuit_free(vc_circuit *c) {
     delete c;
 }
 
+// Fits the bit-field rule of vc_state.cuh to one index array: c = f(0), w_p = f(2^p) - c; every non-zero w_p must be a power
+// of two and consecutive bits with doubling weights form a field (at most three); the rule is then verified on every gate.
+static bool fit_index_rule(const uint32_t *f, uint32_t log_n, uint32_t &mask, uint32_t &c, vc::WireField (&fl)[3]) {
+    c = f[0];
+    uint32_t top = 0;
+    for (uint64_t g = 0; g < (1ull << log_n); g++) top |= f[g];
+    mask = 1; while (mask < top) mask = 2 * mask + 1;          // indices wrap at the smallest power of two above them
+    uint32_t nf = 0;
+    uint32_t p = 0;
+    while (p < log_n) {
+        const uint32_t w = (f[1u << p] - c) & mask;
+        if (w == 0) { p++; continue; }
+        if (w & (w - 1)) return false;
+        uint32_t q0 = 0; while ((1u << q0) != w) q0++;
+        uint32_t len = 1;
+        while (p + len < log_n && q0 + len < 32 && ((f[1u << (p + len)] - c) & mask) == (w << len)) len++;
+        if (nf == 3) return false;
+        fl[nf].p0 = p; fl[nf].m = (uint32_t)((1ull << len) - 1); fl[nf].q0 = q0; fl[nf].pad = 0; nf++;
+        p += len;
+    }
+    const uint64_t n = 1ull << log_n;
+    for (uint64_t g = 0; g < n; g++) {
+        uint32_t v = c;
+        for (uint32_t k = 0; k < 3; k++) v += (((uint32_t)g >> fl[k].p0) & fl[k].m) << fl[k].q0;
+        if ((v & mask) != f[g]) return false;
+    }
+    return true;
+}
+static bool fit_wire_rule(const vc_layer &L, uint32_t log_below, vc::WireRule &r) {
+    const uint32_t ln = L.log_size;
+    if (ln == 0 || log_below > 31) return false;
+    const uint64_t n = 1ull << ln;
+    r = vc::WireRule{};
+    r.t[0] = L.type[0]; r.t[1] = L.type[n - 1]; r.tbit = 0; r.tm = 0;
+    bool one = true, lanes = true;
+    for (uint64_t g = 0; g < n; g++) {
+        one = one && L.type[g] == r.t[0];
+        lanes = lanes && L.type[g] == r.t[(g >> (ln - 1)) & 1];
+    }
+    if (!one) { if (!lanes) return false; r.tbit = ln - 1; r.tm = 1; }
+    return fit_index_rule(L.in1, ln, r.mask[0], r.c[0], r.f[0]) && fit_index_rule(L.in2, ln, r.mask[1], r.c[1], r.f[1]);
+}
+
 static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit *c) {
     int dev = 0, ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
@@ -79,7 +123,7 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
     c->logs[d] = log_input;
     for (uint32_t i = 0; i <= d; i++) if (c->logs[i] > 30) return VC_ERR_SHAPE;
     for (uint32_t i = 1; i <= d; i++) if (c->logs[i] == 0) return VC_ERR_SHAPE;   // a layer below of size 1
-    c->h_type.resize(d); c->h_in1.resize(d); c->h_in2.resize(d); c->wiring.assign(d, 0);
+    c->h_type.resize(d); c->h_in1.resize(d); c->h_in2.resize(d); c->wiring.assign(d, 0); c->wrule.assign(d, vc::WireRule{});
     uint64_t max_gates = 1, max_tab = 2, total = 0;
     size_t part = (size_t)vc::MAX_PART_BLOCKS * 3;
     for (uint32_t i = 0; i < d; i++) {
@@ -94,6 +138,8 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
             onetype = onetype && L.type[g] == L.type[0];
         }
         c->wiring[i] = !onetype ? 0u : (tree ? 1u : (self ? 2u : 0u));
+        const bool no_rule = getenv("VC_NO_WIRE_RULE") != nullptr;     // read at every load: records are read unless tree / self
+        if (c->wiring[i] == 0 && !no_rule && fit_wire_rule(L, c->logs[i + 1], c->wrule[i])) c->wiring[i] = 3u;
         c->h_type[i].assign(L.type, L.type + n);
         c->h_in1[i].assign(L.in1, L.in1 + n);
         c->h_in2[i].assign(L.in2, L.in2 + n);
@@ -308,6 +354,12 @@ extern "C" int vc_debug_layer_stamps(const vc_circuit *c, uint64_t *h_ns, void *
 extern "C" int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind) {
     if (!c || !h_kind) return VC_ERR_ARG;
     return vc::fused_layer_kinds(c, h_kind);
+}
+
+extern "C" int vc_debug_layer_wiring(const vc_circuit *c, uint32_t *h_mode) {
+    if (!c || !h_mode) return VC_ERR_ARG;
+    for (uint32_t i = 0; i < c->d; i++) h_mode[i] = c->wiring[i];
+    return VC_OK;
 }
 
 extern "C" int vc_debug_trace(const vc_circuit *c, uint64_t *h_words, uint32_t n_words, void *cuda_stream) {

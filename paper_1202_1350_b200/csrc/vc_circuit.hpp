@@ -20,9 +20,10 @@ struct vc_circuit {
     std::vector<uint8_t *> d_type;
     std::vector<uint32_t *> d_in1, d_in2;
     std::vector<uint64_t *> d_V;                // d+1 tables, V[d] = input copy
-    // per-layer wiring class (set at load) of layers with a single gate type: 1 = tree (in1 = 2g, in2 = 2g+1),
-    // 2 = self (in1 = in2 = g), else 0 = generic (records are read)
+    // per-layer wiring class (set at load): 1 = tree (in1 = 2g, in2 = 2g+1), 2 = self (in1 = in2 = g), both with a single
+    // gate type; 3 = bit-field rule (wrule[i]); else 0 = generic (records are read)
     std::vector<uint32_t> wiring;
+    std::vector<vc::WireRule> wrule;
     // scratch
     uint64_t *d_P = nullptr;                    // weights, max layer size
     uint64_t *d_T0 = nullptr, *d_T1 = nullptr;  // fold ping-pong

@@ -56,6 +56,8 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
         const uint32_t s = a.L[layer + 1].log_n;
         if (blockIdx.x == 0 && tid == 0) a.stamps[layer] = globaltimer_ns();
         VC_TR(100 + layer);
+        if (tid < sizeof(WireRule) / 4) reinterpret_cast<uint32_t *>(&cx.wrule)[tid] = reinterpret_cast<const uint32_t *>(&a.L[layer].rule)[tid];
+        __syncthreads();
         if (a.L[layer].kind == 0) {
             if (MASK & 1) { if (blockIdx.x == 0) small_layer(a, cx, invfact, pas, dyn, layer, tr); }
             handoff = true;
@@ -430,6 +432,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         lp.V = c->d_V[i];
         lp.log_n = c->logs[i];
         lp.wiring = i < c->d ? c->wiring[i] : W_GENERIC;
+        if (i < c->d) lp.rule = c->wrule[i];
         lp.type0 = i < c->d ? c->h_type[i][0] : 0;
         if (i < c->d) {
             std::vector<CtaPlan> cta;

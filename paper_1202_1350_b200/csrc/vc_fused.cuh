@@ -50,7 +50,8 @@ struct LayerPlan {
     uint32_t thin;                       // != 0: at most one gate per worker thread: vc_fused_thin.cuh; the value = lanes per gate (1 or 4)
     uint32_t resident;                   // 1: gate state in shared memory, 0: in global scratch
     uint32_t has_relay;                  // 1: the layer has RELAY gates (their x is ignored in phase 2)
-    uint32_t wiring, type0;              // implicit wiring (W_TREE / W_SELF with the single gate type type0) or W_GENERIC
+    uint32_t wiring, type0;              // implicit wiring (W_TREE / W_SELF with the single gate type type0, W_FIELDS with `rule`) or W_GENERIC
+    WireRule rule;
     uint32_t cap;                        // state capacity in gates (multiple of FT)
     uint32_t mode[2];                    // per phase: F_MODE_SLICE / F_MODE_GLOBAL
     uint32_t K[2];                       // per phase: first fully shared level
@@ -61,23 +62,38 @@ struct LayerPlan {
 };
 
 // Implicit wiring (§5.2: for regular circuits the in-neighbours of gate g are
-// computed from g instead of being read).  Layers with one gate type whose records are in1 = 2g, in2 = 2g+1 (the add
-// trees) or in1 = in2 = g (the squaring layers) are recognised at load; everything else reads its records.
-constexpr uint32_t W_GENERIC = 0, W_TREE = 1, W_SELF = 2;
+// computed from g instead of being read).  Recognised at load: in1 = 2g, in2 = 2g+1 (the add trees), in1 = in2 = g (the
+// squaring layers), and everything the bit-field rule of vc_state.cuh covers (chain lanes, matrix product, sliding
+// window); everything else reads its records.
+constexpr uint32_t W_GENERIC = 0, W_TREE = 1, W_SELF = 2, W_FIELDS = 3;
 struct Wires {
     const uint8_t *type;
     const uint32_t *in1, *in2;
+    const WireRule *rule;
     uint32_t mode, t0;
-    __device__ __forceinline__ explicit Wires(const LayerPlan &L) : type(L.type), in1(L.in1), in2(L.in2), mode(L.wiring), t0(L.type0) {}
+    __device__ __forceinline__ explicit Wires(const LayerPlan &L) : type(L.type), in1(L.in1), in2(L.in2), rule(&L.rule), mode(L.wiring), t0(L.type0) {}
+    // with the rule read from a copy (shared memory) instead of the plan in global memory
+    __device__ __forceinline__ Wires(const LayerPlan &L, const WireRule *r) : type(L.type), in1(L.in1), in2(L.in2), rule(r), mode(L.wiring), t0(L.type0) {}
+    __device__ __forceinline__ uint32_t field_index(uint32_t g, int which) const {
+        uint32_t v = rule->c[which];
+#pragma unroll
+        for (uint32_t k = 0; k < 3; k++) {
+            const uint4 f = *reinterpret_cast<const uint4 *>(&rule->f[which][k]);     // p0, m, q0
+            v += ((g >> f.x) & f.y) << f.z;
+        }
+        return v & rule->mask[which];
+    }
+    __device__ __forceinline__ uint32_t field_type(uint32_t g) const { return rule->t[(g >> rule->tbit) & rule->tm]; }
     __device__ __forceinline__ void get(uint32_t g, uint32_t &i1, uint32_t &i2, uint32_t &t) const {
         if (mode == W_TREE) { i1 = 2 * g; i2 = 2 * g + 1; t = t0; }
         else if (mode == W_SELF) { i1 = g; i2 = g; t = t0; }
+        else if (mode == W_FIELDS) { i1 = field_index(g, 0); i2 = field_index(g, 1); t = field_type(g); }
         else { i1 = __ldg(in1 + g); i2 = __ldg(in2 + g); t = __ldg(type + g); }
     }
     // one field at a time (the non-resident gate loop needs in1 alone in phase 1, in2 and the type in phase 2)
-    __device__ __forceinline__ uint32_t in1_of(uint32_t g) const { return mode == W_TREE ? 2 * g : (mode == W_SELF ? g : __ldg(in1 + g)); }
-    __device__ __forceinline__ uint32_t in2_of(uint32_t g) const { return mode == W_TREE ? 2 * g + 1 : (mode == W_SELF ? g : __ldg(in2 + g)); }
-    __device__ __forceinline__ uint32_t type_of(uint32_t g) const { return mode == W_GENERIC ? __ldg(type + g) : t0; }
+    __device__ __forceinline__ uint32_t in1_of(uint32_t g) const { return mode == W_TREE ? 2 * g : (mode == W_SELF ? g : (mode == W_FIELDS ? field_index(g, 0) : __ldg(in1 + g))); }
+    __device__ __forceinline__ uint32_t in2_of(uint32_t g) const { return mode == W_TREE ? 2 * g + 1 : (mode == W_SELF ? g : (mode == W_FIELDS ? field_index(g, 1) : __ldg(in2 + g))); }
+    __device__ __forceinline__ uint32_t type_of(uint32_t g) const { return mode == W_GENERIC ? __ldg(type + g) : (mode == W_FIELDS ? field_type(g) : t0); }
 };
 
 struct FusedArgs {
@@ -100,6 +116,8 @@ struct FusedCtx {            // block-shared bookkeeping, replicated in every CT
     uint64_t G[4];
     uint64_t seed, ctr, claim, v1, v2;
     uint32_t epoch, pad;
+    WireRule wrule;          // the current layer's bit-field wiring rule (copied from its plan when the layer starts)
+    uint32_t pad2;
 };
 
 // fixed part of the dynamic shared memory: FusedCtx, then 1/k! for k <= MAX_VARS, then Pascal's triangle C(n,k),

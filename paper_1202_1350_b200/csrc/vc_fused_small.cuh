@@ -40,7 +40,7 @@ __device__ __forceinline__ void small_layer(const FusedArgs &a, FusedCtx &cx, co
     const bool live = tid < n;
     uint64_t P = live ? eq_direct(tid, cx.z, 0, si) : 0;         // a3: beta(z, g) by direct product
     uint32_t i1 = 0, i2 = 0, t = VC_RELAY;
-    if (live) Wires(a.L[layer]).get(tid, i1, i2, t);
+    if (live) Wires(a.L[layer], &cx.wrule).get(tid, i1, i2, t);
     uint32_t ctr = (uint32_t)cx.ctr;
     const uint64_t seed = cx.seed;
     __syncthreads();

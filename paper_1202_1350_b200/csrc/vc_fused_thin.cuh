@@ -52,7 +52,7 @@ __device__ __forceinline__ void thin_layer(const FusedArgs &a, FusedCtx &cx, con
     uint64_t W = 0, cP = fp61::P, P = 0;             // P: the plain weight beta(z,g) eq(low bits of in1[g], r1[0..j)), tracked in phase 1
     uint64_t other = 0;
     if (act) {                                       // the gate's record and fixed operand travel while the eq table is built
-        Wires(Lp).get(g, i1, i2, t);
+        Wires(Lp, &cx.wrule).get(g, i1, i2, t);
         other = __ldg(Vb + i2);
     }
     const EqTab eb = build_eq_tab(bufX, bufX + (1u << F_EQLOG), scr, cx.z, si, tid, FT);

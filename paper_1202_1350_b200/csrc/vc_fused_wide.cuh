@@ -258,7 +258,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     __syncthreads();
     uint64_t claim_part = 0;
     auto setup1 = [&](auto resident) {
-        const Wires wr(Lp);                      // records, or the rule that replaces them (built outside the loop: Lp sits in global memory)
+        const Wires wr(Lp, &cx.wrule);                      // records, or the rule that replaces them (built outside the loop: Lp sits in global memory)
 #pragma unroll 2
         for (uint32_t k = 0; k < nk; k++) {
             const uint32_t l = k * FT + tid;
@@ -302,7 +302,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             const EqTab e1 = build_eq_tab(bufX + (2u << F_EQLOG), bufX + (3u << F_EQLOG), scr + 128, cx.r1, s, tid, FT);
             __syncthreads();
             auto setup2 = [&](auto resident) {
-                const Wires wr(Lp);
+                const Wires wr(Lp, &cx.wrule);
 #pragma unroll 2
                 for (uint32_t k = 0; k < nk; k++) {
                     const uint32_t l = k * FT + tid;
@@ -397,7 +397,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                     } else if (has_ign) hot_gates<true>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                     else hot_gates<false>(upd, sW, sC, sI, tab - base, j, nmine, tid, r_prev, omr, s4);
                 } else {
-                    const Wires wr(Lp);
+                    const Wires wr(Lp, &cx.wrule);
                     for (uint32_t k = 0; k < nmine; k++) {
                         const uint32_t l = k * GT + tid, g = g0 + l;
                         GateIn A;
@@ -405,7 +405,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
                         else {
                             A.W = a.P[g]; A.cP = a.C[g];
                             if (wr.mode == W_GENERIC) A.idx = ph == 0 ? wr.in1[g] : (wr.in2[g] | ((wr.type[g] == VC_RELAY ? 1u : 0u) << 31));
-                            else A.idx = ph == 0 ? wr.in1_of(g) : (wr.in2_of(g) | ((wr.t0 == VC_RELAY ? 1u : 0u) << 31));
+                            else A.idx = ph == 0 ? wr.in1_of(g) : (wr.in2_of(g) | ((wr.type_of(g) == VC_RELAY ? 1u : 0u) << 31));
                         }
                         const uint32_t u = (A.idx & F_IDX_MASK) >> (j + 1);
                         ulonglong2 pr;

@@ -29,4 +29,18 @@ struct DevState {
     uint64_t invfact[MAX_VARS + 1];  // 1/k! mod p, written once at load (Lagrange denominators)
 };
 
+// Implicit wiring by bit fields (for regular circuits the in-neighbours of a gate
+// are "determined with very little arithmetic and no global memory accesses").  An index is
+//     in(g) = ( c + sum_f ((g >> p0_f) & (2^len_f - 1)) << q0_f ) & mask,      at most three fields per index,
+// which covers the add trees (in = 2g, 2g+1), the squaring layers (g), the two lanes of the square-and-multiply chain
+// (g', g' + n by lane), the matrix-product layer (i m + k, m^2 + k m + j from g = (i m + j) m + k) and the sliding window
+// of the pattern matcher ((i + j) mod T, T + j from g = i Q + j).  The gate type is t[bit tbit of g] (two lanes) or t[0].
+// Unpacked so that the device evaluates a field in four instructions: m = 2^len - 1, and an unused field has m = 0.
+struct WireField { uint32_t p0, m, q0, pad; };
+struct alignas(16) WireRule {
+    WireField f[2][3];
+    uint32_t c[2], mask[2];             // mask[w] = 2^k - 1, the smallest that holds every index of operand w (a cyclic window wraps at it)
+    uint32_t t[2], tbit, tm;             // type = t[(g >> tbit) & tm]; tm = 0: one type
+};
+
 }  // namespace vc

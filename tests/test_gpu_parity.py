@@ -334,6 +334,39 @@ def test_cluster_engine_and_grid_kernels_give_the_same_transcript(vc, monkeypatc
     monkeypatch.delenv("VC_NO_CLUSTER")
 
 
+def test_computed_wiring_covers_the_paper_circuits_and_changes_no_word(vc, monkeypatch):
+    """SURVEY.md §8f NEXT-4 (§5.1.4: indices computed, no record loads).  vc_load fits tree / self / bit-field
+    rules to the records; every layer of the four paper circuits gets a computed mode, a random circuit gets none, and with the
+    rule switched off (VC_NO_WIRE_RULE=1: those layers read their records) both schedules give the oracle's words either way.
+    Sizes put the rule through the cluster engine, the thin and the wide kernels (the product layer is 2^15 gates, the
+    sliding-window layer 2^14, the chain lanes 2^14)."""
+    cases = [(W.f0_circuit(13, 5), 61), (W.matmul_circuit(5, 6), 62), (W.pm_circuit(11, 3, 7, planted=3), 63),
+             (W.f2_circuit(12, 8), 64)]
+    for c, seed in cases:
+        want_out, want_tr, _, want_claim = oracle.OracleCircuit(c).prove(c.input, seed)
+        for off in ("", "1"):
+            if off:
+                monkeypatch.setenv("VC_NO_WIRE_RULE", off)
+            else:
+                monkeypatch.delenv("VC_NO_WIRE_RULE", raising=False)
+            for schedule in (0, 1):
+                gc, out, tr = _gpu_prove(vc, c, seed, schedule=schedule)
+                modes = gc.layer_wiring()
+                if off:
+                    assert not (modes == 3).any(), c.name
+                else:
+                    assert (modes != 0).all(), (c.name, modes)
+                    assert c.name.startswith("F2") or (modes == 3).any(), (c.name, modes)
+                assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (c.name, off, schedule)
+                assert gc.state()[1] == want_claim
+                gc.close()
+    monkeypatch.delenv("VC_NO_WIRE_RULE", raising=False)
+    c = W.random_circuit([3, 9, 12, 11], 10, 65)
+    gc = vc.Circuit(c)
+    assert (gc.layer_wiring() == 0).all()
+    gc.close()
+
+
 def test_run_host_end_to_end_matches(vc):
     import torch
     c = W.config(1)
