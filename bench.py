@@ -199,7 +199,8 @@ def run_ours(args):
         kind, n = args.paper_scale.split(":")
         n = int(n)
         c = {"f2": lambda: circuits.f2_circuit(n, W.data_seed(2)), "f0": lambda: circuits.f0_circuit(n, W.data_seed(3)),
-             "matmul": lambda: circuits.matmul_circuit(n, W.data_seed(4)), "pm": lambda: circuits.pm_circuit(n, 3, W.data_seed(5))}[kind]()
+             "matmul": lambda: circuits.matmul_circuit(n, W.data_seed(4)),
+             "matmuleq": lambda: circuits.matmul_eq_circuit(n, W.data_seed(4)), "pm": lambda: circuits.pm_circuit(n, 3, W.data_seed(5))}[kind]()
         k = 0
     from paper_1202_1350_b200 import replicas
     c.input = replicas.replica_input(c.input, W.data_seed(k or 2), rank)   # replicas: same circuit, another seeded input
@@ -420,7 +421,7 @@ def main():
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")
-    ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
+    ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | matmuleq:LOG_M (the single-output circuit of PAPER.md:230) | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
     args = ap.parse_args()
     if args.impl == "reference":

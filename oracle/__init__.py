@@ -76,7 +76,9 @@ def lib():
         L.orc_prove.restype = C.c_int
         L.orc_prove.argtypes = [vp, u32, u32, vp, u64, vp, vp, u64, vp, vp]
         L.orc_layer_entry.restype = u64
-        L.orc_layer_entry.argtypes = [vp, u32, u64, vp]
+        L.orc_layer_entry.argtypes = [vp, u32, u64, C.c_int, vp]
+        L.orc_prove_sum_layer.restype = C.c_int
+        L.orc_prove_sum_layer.argtypes = [u32, vp, u64, vp, vp, vp, vp]
         L.orc_verify.restype = C.c_int
         L.orc_verify.argtypes = [vp, u32, u32, vp, vp, u64, vp, u64, vp, vp, vp]
         _lib = L
@@ -131,12 +133,25 @@ class OracleCircuit:
         lib().orc_start(_ptr(_u64(V0)), s0, seed, C.byref(ctr), _ptr(z), C.byref(claim))
         return z, int(claim.value), int(ctr.value)
 
+    @property
+    def sum_output(self) -> bool:
+        """Layer 0 is the single large-fan-in sum gate (type code 4)."""
+        L0 = self.c.layers[0]
+        return L0.log_size == 0 and int(L0.type[0]) == 4
+
     def prove_layer(self, i, Vbelow, seed, ctr, z, claim, debug=True):
         """Returns (transcript words, z_out[64], claim_out, ctr_out, LayerDebug)."""
         s = self.log_below(i)
         z = _u64(z).copy()
         if z.size < 64:
             z = np.concatenate([z, np.zeros(64 - z.size, dtype=np.uint64)])
+        if i == 0 and self.sum_output:
+            tr = np.zeros(2 * s, dtype=np.uint64)
+            c_ctr, c_claim = C.c_uint64(ctr), C.c_uint64(claim)
+            rc = lib().orc_prove_sum_layer(s, _ptr(_u64(Vbelow)), seed, C.byref(c_ctr), _ptr(z), C.byref(c_claim), _ptr(tr))
+            if rc:
+                raise ValueError(f"orc_prove_sum_layer rc={rc}")
+            return tr, z, int(c_claim.value), int(c_ctr.value), None
         tr = np.zeros(7 * s + 1, dtype=np.uint64)
         c_ctr, c_claim = C.c_uint64(ctr), C.c_uint64(claim)
         dbg = LayerDebug()
@@ -175,7 +190,7 @@ class OracleCircuit:
         """Entry state (z, claim, counter) of layer i in isolation: orc_layer_entry for the point, orc_mle for the claim."""
         logs = np.array([l.log_size for l in self.c.layers] + [self.log_input], dtype=np.uint32)
         zz = np.zeros(64, dtype=np.uint64)
-        ctr = int(lib().orc_layer_entry(logs.ctypes.data_as(C.c_void_p), i, seed, _ptr(zz)))
+        ctr = int(lib().orc_layer_entry(logs.ctypes.data_as(C.c_void_p), i, seed, int(self.sum_output), _ptr(zz)))
         return zz, mle(Vi, zz), ctr
 
 

@@ -21,6 +21,7 @@ from itertools import product
 P = (1 << 61) - 1
 
 ADD, MULT, SUB, RELAY = 0, 1, 2, 3
+SUM = 4     # the single sum gate of large fan-in at the output
 
 
 def chi(b: int, x: int) -> int:
@@ -65,6 +66,9 @@ def evaluate(layers, x):
     for i in range(len(layers) - 1, -1, -1):
         typ, in1, in2 = layers[i]
         below = V[i + 1]
+        if i == 0 and len(typ) == 1 and int(typ[0]) == SUM:       # the output is the sum of EVERY gate of layer 1
+            V[0] = [sum(below) % P]
+            continue
         V[i] = [gate_f(int(typ[g]), below[int(in1[g])], below[int(in2[g])]) for g in range(len(typ))]
     return V
 
@@ -127,3 +131,17 @@ def wiring_sums(layer, z, r1, r2):
     for g in range(len(typ)):
         W[int(typ[g])] += eq(g, z) * eq(int(in1[g]), r1) % P * eq(int(in2[g]), r2)
     return [w % P for w in W]
+
+
+def sum_gate_round_message(Vbelow, prefix, s):
+    """The sum gate of large fan-in (reading c-19): the output is sum_{w Boolean} V~(w), so round m of its
+    sum-check is  g_m(t) = sum over Boolean suffixes b of V~(prefix, t, b),  here for t = 0, 1, 2 (linear in t: the
+    protocol sends t = 0, 1 only; the third value lets a test check the degree)."""
+    m = len(prefix)
+    out = []
+    for t in (0, 1, 2):
+        tot = 0
+        for suffix in product((0, 1), repeat=s - m - 1):
+            tot += mle(Vbelow, list(prefix) + [t] + list(suffix))
+        out.append(tot % P)
+    return out

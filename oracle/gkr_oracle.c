@@ -37,12 +37,12 @@ typedef unsigned __int128 u128;
 
 #define ORC_P ((uint64_t)2305843009213693951ULL) /* 2^61 - 1 */
 
-enum { ORC_ADD = 0, ORC_MULT = 1, ORC_SUB = 2, ORC_RELAY = 3 };
+enum { ORC_ADD = 0, ORC_MULT = 1, ORC_SUB = 2, ORC_RELAY = 3, ORC_SUM = 4 };
 enum { ORC_OK = 0, ORC_ERR_ARG = 1, ORC_ERR_SHAPE = 2, ORC_ERR_NOMEM = 5 };
 
 typedef struct {
     uint32_t log_size;     /* layer has 2^log_size gates */
-    const uint8_t *type;   /* 0 ADD, 1 MULT, 2 SUB, 3 RELAY */
+    const uint8_t *type;   /* 0 ADD, 1 MULT, 2 SUB, 3 RELAY; 4 SUM only as the single gate of layer 0 (see orc_prove_sum_layer) */
     const uint32_t *in1;   /* indices into the layer below */
     const uint32_t *in2;
 } orc_layer;
@@ -121,6 +121,10 @@ uint64_t orc_mle(const uint64_t *V, uint32_t s, const uint64_t *x) {
     return acc;
 }
 
+/* The sum gate of very large fan-in at the output (reading c-19): layer 0 is ONE gate of type SUM whose
+ * in-neighbours are all gates of layer 1 (in1/in2 are not read). */
+static int is_sum_layer(const orc_layer *L) { return L->log_size == 0 && L->type[0] == ORC_SUM; }
+
 /* ---------------------------------------------------------------- evaluation (a1)
  * V[d] <- input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]).
  * V is an array of d+1 caller-allocated buffers. */
@@ -135,6 +139,12 @@ int orc_evaluate(const orc_layer *layers, uint32_t d, uint32_t log_input, const 
         const orc_layer *L = &layers[i];
         uint64_t n = (uint64_t)1 << L->log_size;
         uint64_t nb = (uint64_t)1 << ((uint32_t)i + 1 < d ? layers[i + 1].log_size : log_input);
+        if (i == 0 && is_sum_layer(L)) {            /* y = sum of every value of layer 1 */
+            uint64_t acc = 0;
+            for (uint64_t u = 0; u < nb; u++) acc = orc_add(acc, V[1][u]);
+            V[0][0] = acc;
+            continue;
+        }
         for (uint64_t g = 0; g < n; g++) {
             if (L->type[g] > 3 || L->in1[g] >= nb || L->in2[g] >= nb) return ORC_ERR_SHAPE;
             V[i][g] = gate_f(L->type[g], V[i + 1][L->in1[g]], V[i + 1][L->in2[g]]);
@@ -243,19 +253,54 @@ int orc_prove_layer(const orc_layer *L, uint32_t s, const uint64_t *Vb, uint64_t
     return ORC_OK;
 }
 
+/* ---------------------------------------------------------------- the sum gate at the output (reading c-19)
+ * "The GKR protocol typically assumes that all gates have fan-in two, but [8] explains how the protocol can be modified
+ * to handle a single sum-gate of very large fan-in at the output."  The output is y = sum_{w in {0,1}^s} V_1[w], and V_1[w]
+ * = V~_1(w) on Boolean w, so the claim "y" is a sum of the multilinear V~_1 over the cube: a sum-check over its s variables,
+ * bit 0 first (reading c-2).  Round j:
+ *     g_j(t) = sum over Boolean suffixes b of V~_1(r_0..r_{j-1}, t, b)          (degree 1 in t: sent as g_j(0), g_j(1))
+ *     V checks g_j(0) + g_j(1) = claim, draws r_j, claim <- g_j(r_j) = g_j(0) + r_j (g_j(1) - g_j(0)).
+ * After s rounds the claim is V~_1(r) at ONE point: z' = r, no line restriction and no tau.
+ * A = copy(V_1) is folded by r_j after every round, as in the layer sum-check (a6).  tr: 2 s words; s draws. */
+int orc_prove_sum_layer(uint32_t s, const uint64_t *Vb, uint64_t seed, uint64_t *ctr, uint64_t *z, uint64_t *claim,
+                        uint64_t *tr) {
+    if (s == 0 || s > 63) return ORC_ERR_SHAPE;
+    uint64_t nb = (uint64_t)1 << s, w = 0;
+    uint64_t *A = (uint64_t *)malloc(nb * sizeof(uint64_t));
+    if (!A) return ORC_ERR_NOMEM;
+    memcpy(A, Vb, nb * sizeof(uint64_t));
+    for (uint32_t j = 0; j < s; j++) {
+        uint64_t half = nb >> (j + 1), G0 = 0, G1 = 0;
+        for (uint64_t u = 0; u < half; u++) { G0 = orc_add(G0, A[2 * u]); G1 = orc_add(G1, A[2 * u + 1]); }
+        tr[w++] = G0; tr[w++] = G1;
+        uint64_t r = orc_draw(seed, (*ctr)++);
+        z[j] = r;
+        for (uint64_t u = 0; u < half; u++)
+            A[u] = orc_add(A[2 * u], orc_mul(r, orc_sub(A[2 * u + 1], A[2 * u])));
+    }
+    *claim = A[0];
+    free(A);
+    return ORC_OK;
+}
+
 /* Entry state of layer i taken in isolation.  The challenges are a function of (seed, counter) alone (reading c-11),
  * the counter advances by s_0 for z_0 and by 2 s_{l+1} + 1 per proved layer l (2s round challenges, then tau), and
  * the claim point of layer i >= 1 is z = l(tau) = r1 + tau (r2 - r1) with r1, r2, tau the draws of layer i-1
  * (reading c-5).  logs[0..i] = log sizes of layers 0..i.  Writes z[0 .. logs[i]) and returns the counter at which
  * layer i's own draws start.  (The claim at z is V~_i(z) by definition: orc_mle.) */
-uint64_t orc_layer_entry(const uint32_t *logs, uint32_t i, uint64_t seed, uint64_t *z) {
+uint64_t orc_layer_entry(const uint32_t *logs, uint32_t i, uint64_t seed, int sum_out, uint64_t *z) {
     if (i == 0) {
         for (uint32_t k = 0; k < logs[0]; k++) z[k] = orc_draw(seed, k);
         return logs[0];
     }
+    /* sum_out: layer 0 is the sum gate (s_0 = 0): it takes s_1 draws and hands z = (r_0..r_{s_1 - 1}) to layer 1 */
     uint64_t c0 = logs[0];
-    for (uint32_t l = 0; l + 1 < i; l++) c0 += 2ull * logs[l + 1] + 1;
+    for (uint32_t l = 0; l + 1 < i; l++) c0 += (sum_out && l == 0) ? logs[1] : 2ull * logs[l + 1] + 1;
     const uint32_t s = logs[i];
+    if (sum_out && i == 1) {
+        for (uint32_t k = 0; k < s; k++) z[k] = orc_draw(seed, c0 + k);
+        return c0 + s;
+    }
     const uint64_t tau = orc_draw(seed, c0 + 2ull * s);
     for (uint32_t k = 0; k < s; k++) {
         const uint64_t r1 = orc_draw(seed, c0 + k), r2 = orc_draw(seed, c0 + s + k);
@@ -268,9 +313,15 @@ static uint32_t log_below(const orc_layer *layers, uint32_t d, uint32_t log_inpu
     return i + 1 < d ? layers[i + 1].log_size : log_input;
 }
 
+/* words layer i writes: (G0,G1,G2) x 2s rounds, then q[0..s]; the sum gate: (G0,G1) x s rounds */
+static uint64_t layer_words(const orc_layer *layers, uint32_t d, uint32_t log_input, uint32_t i) {
+    uint64_t s = log_below(layers, d, log_input, i);
+    return (i == 0 && is_sum_layer(&layers[0])) ? 2 * s : 7 * s + 1;
+}
+
 uint64_t orc_transcript_words(const orc_layer *layers, uint32_t d, uint32_t log_input) {
     uint64_t w = 0;
-    for (uint32_t i = 0; i < d; i++) w += 7 * (uint64_t)log_below(layers, d, log_input, i) + 1;
+    for (uint32_t i = 0; i < d; i++) w += layer_words(layers, d, log_input, i);
     return w;
 }
 
@@ -297,8 +348,9 @@ int orc_prove(const orc_layer *layers, uint32_t d, uint32_t log_input, const uin
     }
     for (uint32_t i = 0; i < d && rc == ORC_OK; i++) {
         uint32_t s = log_below(layers, d, log_input, i);
-        rc = orc_prove_layer(&layers[i], s, V[i + 1], seed, &ctr, z, &claim, transcript + w, NULL);
-        w += 7 * (uint64_t)s + 1;
+        if (i == 0 && is_sum_layer(&layers[0])) rc = orc_prove_sum_layer(s, V[1], seed, &ctr, z, &claim, transcript + w);
+        else rc = orc_prove_layer(&layers[i], s, V[i + 1], seed, &ctr, z, &claim, transcript + w, NULL);
+        w += layer_words(layers, d, log_input, i);
     }
     if (rc == ORC_OK && final_z) memcpy(final_z, z, log_input * sizeof(uint64_t));
     if (rc == ORC_OK && final_claim) *final_claim = claim;
@@ -313,7 +365,7 @@ int orc_prove(const orc_layer *layers, uint32_t d, uint32_t log_input, const uin
  * claim == sum_tau W_tau f_tau(v1,v2); then z <- l(tau), claim <- q(tau); at the end
  * claim == V~_d(z) of the input.  Rejection is reported through accept/fail_layer/fail_round:
  * fail_round m < 2s: round check m failed; fail_round = 2s: wiring check failed; fail_layer = d:
- * the closing input check failed. */
+ * the closing input check failed.  A sum gate at the output (reading c-19) has s round checks and nothing else. */
 int orc_verify(const orc_layer *layers, uint32_t d, uint32_t log_input, const uint64_t *input,
                const uint64_t *outputs, uint64_t seed, const uint64_t *transcript, uint64_t n_words,
                int *accept, uint32_t *fail_layer, uint32_t *fail_round) {
@@ -327,6 +379,15 @@ int orc_verify(const orc_layer *layers, uint32_t d, uint32_t log_input, const ui
         uint32_t s = log_below(layers, d, log_input, i);
         uint64_t n = (uint64_t)1 << L->log_size, nb = (uint64_t)1 << s;
         uint64_t r[128];
+        if (i == 0 && is_sum_layer(L)) {      /* the sum gate: s linear rounds, then the claim is V~_1(r) at z = r */
+            for (uint32_t m = 0; m < s; m++) {
+                const uint64_t *G = transcript + w; w += 2;
+                if (orc_add(G[0], G[1]) != claim) { *fail_layer = 0; *fail_round = m; return ORC_OK; }
+                z[m] = orc_draw(seed, ctr++);
+                claim = orc_add(G[0], orc_mul(z[m], orc_sub(G[1], G[0])));
+            }
+            continue;
+        }
         for (uint32_t m = 0; m < 2 * s; m++) {
             const uint64_t *G = transcript + w; w += 3;
             if (orc_add(G[0], G[1]) != claim) { *fail_layer = i; *fail_round = m; return ORC_OK; }

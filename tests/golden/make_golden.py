@@ -1,7 +1,7 @@
 """Writes tests/golden/config<k>.txt and tests/golden/paper_<kind>_<n>.txt from the CPU oracle ONLY (never from the CUDA path).
 
     python tests/golden/make_golden.py 1 2 3 4 5                  # BASELINE.json configs
-    python tests/golden/make_golden.py f2:22 f2:23 matmul:8 pm:19 f0:20   # paper-scale constructions
+    python tests/golden/make_golden.py f2:22 f2:23 matmul:8 matmuleq:8 pm:19 f0:20 f0:21   # paper-scale constructions
 
 For BASELINE.json config k (data seed 1000+k, challenge seed 2000+k; DESIGN.md input recipe) the
 oracle (oracle/gkr_oracle.c, single thread) evaluates the circuit and produces the honest transcript;
@@ -31,14 +31,15 @@ def sha(a: np.ndarray) -> str:
 
 
 # paper-scale cases: (data seed, challenge seed) are the ones tests/test_gpu_verifier.py uses
-PAPER_SEEDS = {"f2": (7, 31337), "matmul": (4, 4242), "pm": (5, 4242), "f0": (3, 4242)}
+PAPER_SEEDS = {"f2": (7, 31337), "matmul": (4, 4242), "pm": (5, 4242), "f0": (3, 4242), "matmuleq": (4, 4242)}
 
 
 def paper_case(kind: str, n: int):
     from vc_workloads import circuits
     ds, cs = PAPER_SEEDS[kind]
     c = {"f2": lambda: circuits.f2_circuit(n, ds), "matmul": lambda: circuits.matmul_circuit(n, ds),
-         "pm": lambda: circuits.pm_circuit(n, 3, ds), "f0": lambda: circuits.f0_circuit(n, ds)}[kind]()
+         "pm": lambda: circuits.pm_circuit(n, 3, ds), "f0": lambda: circuits.f0_circuit(n, ds),
+         "matmuleq": lambda: circuits.matmul_eq_circuit(n, ds, wrong=3)}[kind]()
     return c, cs
 
 

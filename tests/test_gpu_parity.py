@@ -367,6 +367,23 @@ def test_computed_wiring_covers_the_paper_circuits_and_changes_no_word(vc, monke
     gc.close()
 
 
+@pytest.mark.parametrize("log_m,wrong", [(3, 0), (4, 2), (5, 1)])
+def test_matmul_equality_circuit_single_output_bit_exact(vc, log_m, wrong):
+    """The paper's single-output MATMULT circuit, element by element against the
+    oracle on both schedules: mixed MULT / SUB product layer with irregular wiring (records are read), log m + 1 tree
+    layers, the ^(p-1) chain, the counting tree.  The output is the number of wrong entries of C (0 iff C = AB)."""
+    c = W.matmul_eq_circuit(log_m, 30 + log_m, wrong)
+    seed = 70 + log_m
+    want_out, want_tr, _, want_claim = oracle.OracleCircuit(c).prove(c.input, seed)
+    assert want_out.size == 1 and int(want_out[0]) == wrong
+    for schedule in (0, 1):
+        gc, out, tr = _gpu_prove(vc, c, seed, schedule=schedule)
+        assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (log_m, schedule)
+        assert gc.state()[1] == want_claim
+        assert gc.verify(c.input, out, seed, tr) == (True, 0, 0)
+        gc.close()
+
+
 def test_run_host_end_to_end_matches(vc):
     import torch
     c = W.config(1)

@@ -210,16 +210,17 @@ def test_paper_scale_f2_runs_and_verifies(vc):
     gc.close()
 
 
-@pytest.mark.parametrize("kind,n", [("matmul", 8), ("pm", 19), ("f0", 20)])
+@pytest.mark.parametrize("kind,n", [("matmul", 8), ("matmuleq", 8), ("pm", 19), ("f0", 20), ("f0", 21)])
 def test_paper_scale_other_constructions(vc, kind, n):
-    """MATMULT 256 x 256, PM with 2^19 text symbols (Table 2's sizes) and F0 at
-    2^20 (half of Table 2's 2^21: the oracle needs ~20 min and 9 GB for 2^21, and no new code path is reached; bench.py
-    --paper-scale f0:21 times it).  Transcripts are compared with the oracle's per-layer digests
+    """MATMULT 256 x 256 — both the multi-output circuit of BASELINE.json's config 4 and the paper's
+    single-output circuit (AB - C entry by entry, then the F0 circuit; three entries of C are wrong here, so
+    the output is 3) —, PM with 2^19 text symbols and F0 at 2^20 and 2^21 (Table 2's sizes).
+    Transcripts are compared with the oracle's per-layer digests
     (tests/golden/paper_<kind>_<n>.txt); also: outputs equal the directly computed values, the device verifier accepts,
     a flipped word is rejected."""
     from vc_workloads import circuits
     c = {"matmul": lambda: circuits.matmul_circuit(n, 4), "pm": lambda: circuits.pm_circuit(n, 3, 5),
-         "f0": lambda: circuits.f0_circuit(n, 3)}[kind]()
+         "f0": lambda: circuits.f0_circuit(n, 3), "matmuleq": lambda: circuits.matmul_eq_circuit(n, 4, wrong=3)}[kind]()
     gc = vc.Circuit(c)
     gc.set_input(c.input)
     gc.evaluate(); gc.prove(4242)
@@ -227,6 +228,8 @@ def test_paper_scale_other_constructions(vc, kind, n):
     out, tr = gc.outputs().copy(), gc.transcript().copy()
     if kind == "matmul":
         assert np.array_equal(out.reshape(c.meta["A"].shape), c.meta["A"] @ c.meta["B"])          # entries < 2^28: no wrap
+    elif kind == "matmuleq":
+        assert out.size == 1 and int(out[0]) == 3 == int(np.count_nonzero(c.meta["A"] @ c.meta["B"] != c.meta["C"]))
     elif kind == "pm":
         T, Q = c.meta["text"].size, c.meta["pattern"].size
         idx = (np.arange(T)[:, None] + np.arange(Q)[None, :]) % T

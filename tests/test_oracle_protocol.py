@@ -205,3 +205,66 @@ def test_boolean_claim_point_reduces_to_one_gate():
         want = [D.chi(bit, t) * D.gate_f(typ, (lo + t * (hi - lo)) % P, w) % P for t in (0, 1, 2)]
         assert G == want
         assert (G[0] + G[1]) % P == claim
+
+
+# ------------------------------------------------------------------ the sum gate of large fan-in at the output (c-19)
+@pytest.mark.parametrize("s,seed", [(1, 3), (3, 4), (5, 5)])
+def test_sum_gate_rounds_equal_the_definition(s, seed):
+    """Every message of orc_prove_sum_layer against the exponential sum of gkr_def.sum_gate_round_message on a random table
+    of F_p words; the messages are linear in t (two words suffice); the claim chain; the point and the counter."""
+    rng = random.Random(seed)
+    Vb = np.array([rng.randrange(P) for _ in range(1 << s)], dtype=np.uint64)
+    typ = np.array([W.SUM], np.uint8); z0 = np.zeros(1, np.uint32)
+    c = W.Circuit([W.Layer(0, typ, z0, z0)], s, Vb, "sum gate alone")
+    oc = oracle.OracleCircuit(c)
+    assert oc.sum_output and c.sum_output and c.total_transcript_words == 2 * s == oc.transcript_words()
+    y = sum(int(v) for v in Vb) % P
+    assert int(oc.evaluate(Vb)[0][0]) == y == D.evaluate([(typ, z0, z0)], Vb)[0][0]
+    tr, z, claim, ctr, _ = oc.prove_layer(0, Vb, 500 + seed, 0, np.zeros(64, np.uint64), y)
+    chal = [oracle.draw(500 + seed, k) for k in range(s)]
+    assert ctr == s and [int(v) for v in z[:s]] == chal            # z' = r: one point, no line restriction, no tau
+    cur = y
+    for m in range(s):
+        want = D.sum_gate_round_message([int(v) for v in Vb], chal[:m], s)
+        G = [int(v) for v in tr[2 * m:2 * m + 2]]
+        assert G == want[:2], m
+        assert want[2] == (2 * want[1] - want[0]) % P            # degree 1 in t
+        assert (G[0] + G[1]) % P == cur
+        cur = (G[0] + chal[m] * (G[1] - G[0])) % P
+    assert claim == cur == D.mle([int(v) for v in Vb], chal) == oracle.mle(Vb, z)
+
+
+def test_sum_gate_circuits_chain_verify_and_reject_tampering():
+    """F2 and F0 as the paper draws them (one sum gate over the squares / over the ^(p-1) chain): outputs against the direct
+    values, whole prover == layer-wise chain, layer_entry in isolation, honest transcript accepted, every word of the sum
+    gate's rounds and the words of the layer below rejected where predicted."""
+    for c, seed in [(W.f2_sum_circuit(4, 11), 91), (W.f0_sum_circuit(3, 12), 92)]:
+        oc, V, recs, (zf, claimf, _) = _run_layers(c, seed)
+        direct = sum(int(a) * int(a) for a in c.input) % P if c.name.startswith("F2") else int(np.count_nonzero(c.input))
+        assert V[0].size == 1 and int(V[0][0]) == direct
+        out, tr, fz, fc = oc.prove(c.input, seed)
+        assert np.array_equal(tr, np.concatenate([r["tr"] for r in recs])) and fc == claimf
+        assert tr.size == c.total_transcript_words == oc.transcript_words()
+        for rec in recs:
+            z, claim, ctr = oc.layer_entry(rec["i"], seed, V[rec["i"]])
+            assert [int(v) for v in z[:len(rec["z"])]] == rec["z"] and (claim, ctr) == (rec["claim"], rec["ctr"])
+        assert oc.verify(c.input, out, seed, tr) == (True, 0, 0)
+        s = oc.log_below(0)
+        for w in range(2 * s):                                      # G0 or G1 of round w // 2 breaks that round's sum
+            bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+            assert oc.verify(c.input, out, seed, bad) == (False, 0, w // 2)
+        bad = tr.copy(); bad[2 * s] = (int(bad[2 * s]) + 1) % P     # first word of layer 1
+        assert oc.verify(c.input, out, seed, bad) == (False, 1, 0)
+        assert oc.verify(c.input, (out + np.uint64(1)) % np.uint64(P), seed, tr) == (False, 0, 0)
+        bad_in = c.input.copy(); bad_in[1] = (int(bad_in[1]) + 1) % P
+        assert oc.verify(bad_in, out, seed, tr) == (False, c.d, 0)
+
+
+def test_sum_gate_and_add_tree_reach_the_same_output():
+    """The sum gate replaces the binary add tree of BASELINE.json's configs: same value, fewer layers."""
+    a, b = W.f2_circuit(6, 9), W.f2_sum_circuit(6, 9)
+    assert np.array_equal(a.input, b.input) and (a.d, b.d) == (7, 2)
+    assert oracle.OracleCircuit(a).evaluate(a.input)[0][0] == oracle.OracleCircuit(b).evaluate(b.input)[0][0]
+    a, b = W.f0_circuit(4, 9), W.f0_sum_circuit(4, 9)
+    assert (a.d, b.d) == (123, 120)
+    assert oracle.OracleCircuit(a).evaluate(a.input)[0][0] == oracle.OracleCircuit(b).evaluate(b.input)[0][0]

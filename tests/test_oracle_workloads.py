@@ -94,6 +94,20 @@ def test_matmul_outputs_are_the_product():
     assert np.array_equal(c.input[:128 * 128].reshape(128, 128), c.meta["A"])
 
 
+@pytest.mark.parametrize("wrong", [0, 1, 7])
+def test_matmul_equality_circuit_has_one_output_that_counts_wrong_entries(wrong):
+    """a single output gate, zero iff C = AB (the F0 circuit counts the non-zero entries of AB - C)."""
+    c = W.matmul_eq_circuit(3, 21, wrong)
+    V = oracle.OracleCircuit(c).evaluate(c.input)
+    assert V[0].size == 1 and int(V[0][0]) == wrong
+    A, B, Cc = (c.meta[k].astype(object) for k in "ABC")
+    diff = (A.dot(B) - Cc) % P                               # exact Python ints
+    lay = c.d - 1 - 4                                       # below it: the product layer and the 3 + 1 tree layers over the 2m terms
+    assert np.array_equal(V[lay].reshape(8, 8), np.array(diff, dtype=np.uint64))
+    assert int(np.count_nonzero(diff)) == wrong and c.meta["wrong"].size == wrong
+    assert c.input.size == 4 * 64 and not c.input[3 * 64:].any()
+
+
 @pytest.mark.slow
 def test_pm_output_counts_nonmatching_cyclic_offsets():
     c = W.config(5)

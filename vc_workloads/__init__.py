@@ -7,7 +7,7 @@ their circuits and inputs from here, so that the two implementations see identic
 while sharing no code.  Recipes: DESIGN.md "Input recipe"; shapes: BASELINE.json configs.
 """
 from .circuits import (  # noqa: F401
-    ADD, MULT, SUB, RELAY, Circuit, Layer,
-    f2_circuit, f0_circuit, matmul_circuit, pm_circuit, random_circuit,
+    ADD, MULT, SUB, RELAY, SUM, Circuit, Layer,
+    f2_circuit, f0_circuit, matmul_circuit, matmul_eq_circuit, pm_circuit, f2_sum_circuit, f0_sum_circuit, random_circuit,
     config, CONFIG_NAMES, data_seed, challenge_seed,
 )

@@ -19,6 +19,7 @@ from typing import List
 import numpy as np
 
 ADD, MULT, SUB, RELAY = 0, 1, 2, 3
+SUM = 4     # the single sum gate of very large fan-in at the output; only as layer 0, log_size 0
 
 CONFIG_NAMES = {
     1: "F2 n=2^10",
@@ -68,14 +69,21 @@ class Circuit:
 
     @property
     def rounds(self) -> int:
-        return sum(2 * self.log_below(i) for i in range(self.d))
+        return sum((1 if (i == 0 and self.sum_output) else 2) * self.log_below(i) for i in range(self.d))
 
     @property
     def gate_rounds(self) -> int:
-        return sum((1 << self.layers[i].log_size) * 2 * self.log_below(i) for i in range(self.d))
+        return sum((1 << self.layers[i].log_size) * (1 if (i == 0 and self.sum_output) else 2) * self.log_below(i)
+                   for i in range(self.d))
+
+    @property
+    def sum_output(self) -> bool:
+        """Layer 0 is the single sum gate of large fan-in (type code SUM)."""
+        return self.layers[0].log_size == 0 and int(self.layers[0].type[0]) == SUM
 
     def transcript_words(self, i: int) -> int:
-        return 7 * self.log_below(i) + 1
+        """Words layer i writes: (G0,G1,G2) per round for 2s rounds, then q[0..s]; the sum gate: (G0,G1) for s rounds."""
+        return 2 * self.log_below(i) if (i == 0 and self.sum_output) else 7 * self.log_below(i) + 1
 
     @property
     def total_transcript_words(self) -> int:
@@ -134,6 +142,25 @@ def f2_circuit(log_n: int, seed: int) -> Circuit:
     return Circuit(layers_in_first[::-1], log_n, x, f"F2 n=2^{log_n}")
 
 
+def _sum_gate() -> Layer:
+    """Layer 0 of the paper's own F2 / F0 circuits: one gate that sums EVERY gate of layer 1 (reading c-19).
+    in1 / in2 are placeholders (never read)."""
+    return _layer(0, SUM, np.zeros(1, np.uint32), np.zeros(1, np.uint32))
+
+
+def f2_sum_circuit(log_n: int, seed: int) -> Circuit:
+    """F2 exactly as the paper draws it (Fig. 4): a layer of squaring gates, then one sum gate of fan-in n
+    (instead of BASELINE.json's log n-layer binary add tree).  Same input recipe as f2_circuit."""
+    base = f2_circuit(log_n, seed)
+    return Circuit([_sum_gate(), base.layers[-1]], log_n, base.input, f"F2-sum n=2^{log_n}")
+
+
+def f0_sum_circuit(log_n: int, seed: int) -> Circuit:
+    """F0 with the paper's sum gate of high fan-in over the ^(p-1) chain.  Same input recipe as f0_circuit."""
+    base = f0_circuit(log_n, seed)
+    return Circuit([_sum_gate()] + base.layers[log_n:], log_n, base.input, f"F0-sum n=2^{log_n}")
+
+
 def f0_circuit(log_n: int, seed: int) -> Circuit:
     """F0 = #{i : a_i != 0} via a^(p-1) (BASELINE.json configs[2])."""
     rng = np.random.default_rng(seed)
@@ -161,6 +188,42 @@ def matmul_circuit(log_m: int, seed: int) -> Circuit:
     prod = _layer(3 * log_m, MULT, i * m + k, m * m + k * m + j)
     layers_in_first = [prod] + [_tree_layer(t) for t in range(3 * log_m - 1, 2 * log_m - 1, -1)]
     return Circuit(layers_in_first[::-1], 2 * log_m + 1, x, f"MATMUL {m}x{m}", {"A": A, "B": B})
+
+
+def matmul_eq_circuit(log_m: int, seed: int, wrong: int = 0) -> Circuit:
+    """The paper's single-output MATMULT circuit: computes the m^2 entries of AB by
+    naive multiplication, subtracts the claimed C from each, and counts the non-zero differences with the F0 circuit;
+    the one output is 0 iff C = AB.
+
+    Input = A, B, C row-major, then m^2 zeros (4 m^2 = 2^(2 log_m + 2) words); C = AB with `wrong` entries off by one.
+    A layered circuit reads only the layer below, so -C[i,j] enters the sum over k as one more term: the inner dimension
+    is 2m wide, gate g = (i*m + j)*2m + k' is A[i,k']*B[k',j] (MULT) for k' < m, 0 - C[i,j] (SUB) for k' = m and 0 - 0
+    above; log_m + 1 add-tree layers give (AB - C)[i,j]; the ^(p-1) chain and a 2 log_m-layer add tree count the
+    non-zero entries.
+    """
+    rng = np.random.default_rng(seed)
+    m = 1 << log_m
+    A = rng.integers(0, 1 << 10, size=(m, m), dtype=np.uint64)
+    B = rng.integers(0, 1 << 10, size=(m, m), dtype=np.uint64)
+    Cm = A @ B                                               # entries < 2^28: no wrap
+    bad = rng.choice(m * m, size=wrong, replace=False) if wrong else np.zeros(0, dtype=np.int64)
+    Cf = Cm.reshape(-1).copy()
+    Cf[bad] += np.uint64(1)
+    x = np.concatenate([A.reshape(-1), B.reshape(-1), Cf, np.zeros(m * m, dtype=np.uint64)])
+    Z = 3 * m * m                                            # a zero word of the input
+    g = np.arange(2 * m * m * m, dtype=np.uint64)
+    ij, k = g // (2 * m), g % (2 * m)
+    i, j = ij // m, ij % m
+    kk = np.minimum(k, m - 1)
+    in1 = np.where(k < m, i * m + kk, Z)
+    in2 = np.where(k < m, m * m + kk * m + j, np.where(k == m, 2 * m * m + ij, Z))
+    typ = np.where(k < m, MULT, SUB).astype(np.uint8)
+    prod = _layer(3 * log_m + 1, typ, in1, in2)
+    layers_in_first = [prod] + [_tree_layer(t) for t in range(3 * log_m, 2 * log_m - 1, -1)]
+    layers_in_first += _fermat_chain(2 * log_m)
+    layers_in_first += [_tree_layer(t) for t in range(2 * log_m - 1, -1, -1)]
+    return Circuit(layers_in_first[::-1], 2 * log_m + 2, x, f"MATMUL-EQ {m}x{m}",
+                   {"A": A, "B": B, "C": Cf.reshape(m, m), "wrong": np.sort(bad)})
 
 
 def pm_circuit(log_t: int, log_q: int, seed: int, planted: int = 16) -> Circuit:
