@@ -43,6 +43,10 @@ def algorithmic_counts(c):
     for i, L in enumerate(c.layers):
         n, s = 1 << L.log_size, c.log_below(i)
         nb = 1 << s
+        if i == 0 and c.sum_output:      # the sum gate: s rounds over the shrinking table, read 8*2^(s-j) and write half per round
+            per_layer.append(dict(n=1, s=s, prove_bytes=24 * nb, round_bytes=[12 * (nb >> j) for j in range(s)],
+                                  eval_bytes=8 * nb, modmul=nb, modmul_eval=0))
+            continue
         rounds_bytes = n * s * (33 + 25)
         table_bytes = 2 * 24 * nb
         line_bytes = 8 * nb
@@ -200,7 +204,8 @@ def run_ours(args):
         n = int(n)
         c = {"f2": lambda: circuits.f2_circuit(n, W.data_seed(2)), "f0": lambda: circuits.f0_circuit(n, W.data_seed(3)),
              "matmul": lambda: circuits.matmul_circuit(n, W.data_seed(4)),
-             "matmuleq": lambda: circuits.matmul_eq_circuit(n, W.data_seed(4)), "pm": lambda: circuits.pm_circuit(n, 3, W.data_seed(5))}[kind]()
+             "matmuleq": lambda: circuits.matmul_eq_circuit(n, W.data_seed(4)),
+             "f2sum": lambda: circuits.f2_sum_circuit(n, W.data_seed(2)), "f0sum": lambda: circuits.f0_sum_circuit(n, W.data_seed(3)), "pm": lambda: circuits.pm_circuit(n, 3, W.data_seed(5))}[kind]()
         k = 0
     from paper_1202_1350_b200 import replicas
     c.input = replicas.replica_input(c.input, W.data_seed(k or 2), rank)   # replicas: same circuit, another seeded input
@@ -421,7 +426,7 @@ def main():
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")
-    ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | matmuleq:LOG_M (the single-output circuit of PAPER.md:230) | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
+    ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | matmuleq:LOG_M (the single-output circuit of PAPER.md:230) | f2sum:N | f0sum:N (the paper's circuits with ONE sum gate of fan-in n at the output, PAPER.md:220) | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
     args = ap.parse_args()
     if args.impl == "reference":

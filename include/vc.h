@@ -24,12 +24,21 @@ extern "C" {
 typedef struct vc_circuit vc_circuit; /* opaque; owns device copies of records, V tables, scratch, proof state */
 
 enum { VC_OK = 0, VC_ERR_ARG = 1, VC_ERR_SHAPE = 2, VC_ERR_STATE = 3, VC_ERR_CUDA = 4, VC_ERR_NOMEM = 5 };
-enum { VC_ADD = 0, VC_MULT = 1, VC_SUB = 2, VC_RELAY = 3 };
+enum { VC_ADD = 0, VC_MULT = 1, VC_SUB = 2, VC_RELAY = 3, VC_SUM = 4 };
+
+/* VC_SUM — the "single sum-gate of very large fan-in at the output" (DESIGN.md
+ * reading c-19).  Allowed only as the ONE gate of layer 0 (log_size 0; in1 / in2 need one placeholder entry each and are
+ * not read): its in-neighbours are ALL gates of layer 1, V_0[0] = sum_w V_1[w].  Its iteration of the protocol is a
+ * sum-check over the s = log_size(layer 1) variables of the multilinear extension of V_1, bit 0 first: round j emits
+ * (g_j(0), g_j(1)) = the sums of the even- and odd-indexed entries of the table folded by r_0..r_{j-1}, the challenge
+ * r_j is drawn on the device, and after s rounds the claim is V~_1(r) at the one point z' = r (no line restriction, no
+ * tau).  Such a layer writes 2 s transcript words and takes s draws; the verifiers check g_j(0) + g_j(1) = claim and
+ * continue with claim <- g_j(0) + r_j (g_j(1) - g_j(0)): fail_round = j < s, and there is no wiring check for it. */
 
 /* One layer's gate records, structure-of-arrays, in HOST memory (copied at load; caller keeps ownership). */
 typedef struct {
     uint32_t log_size;    /* the layer has exactly 2^log_size gates */
-    const uint8_t *type;  /* VC_ADD L+R, VC_MULT L*R, VC_SUB L-R, VC_RELAY L */
+    const uint8_t *type;  /* VC_ADD L+R, VC_MULT L*R, VC_SUB L-R, VC_RELAY L; VC_SUM only as the single gate of layer 0 (above) */
     const uint32_t *in1;  /* indices into the layer below, < 2^log_size(below) */
     const uint32_t *in2;
 } vc_layer;
@@ -40,11 +49,11 @@ typedef struct {
  * PAPER.md:153 (§5.1.1): the whole circuit stays resident in HBM.
  *   layers[0] = output layer ... layers[d-1] = the layer fed by the input; log_input = log2(#inputs).
  * Errors: VC_ERR_ARG (null, d = 0), VC_ERR_SHAPE (log_size > 30, a layer below of size 1, index out
- * of range, unknown type), VC_ERR_CUDA / VC_ERR_NOMEM. */
+ * of range, unknown type, VC_SUM anywhere but as the single gate of layer 0), VC_ERR_CUDA / VC_ERR_NOMEM. */
 int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit **out);
 
 /* vc_evaluate — layered circuit evaluation (step a1; §6.2.4):
- * V_d = input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]]).
+ * V_d = input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]])  (a VC_SUM output: the sum of V_1).
  *   d_input   DEVICE pointer, 2^log_input canonical words (read).  A word >= p is detected ON THE DEVICE while the input
  *             is copied, i.e. asynchronously: the call itself still returns VC_OK ("enqueued").  The sticky bit 0 of the
  *             status word reports it for THIS evaluation (it is cleared when vc_evaluate is enqueued): vc_status reads
@@ -61,8 +70,9 @@ int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, voi
  * in1, phase 2 the bits of in2, LSB first; each round emits G[0],G[1],G[2] = the round polynomial at
  * t = 0,1,2, reduced mod p over all gates, then draws the challenge on the device), then the line
  * restriction q[0..s] = V~_{i+1}(r1 + t (r2 - r1)), a draw tau, z <- l(tau), claim <- q(tau).
- *   d_transcript DEVICE pointer, receives 7*s+1 words: 2s x (G0,G1,G2), then q[0..s].
- *   cap_words    capacity of d_transcript in words (VC_ERR_ARG if < 7*s+1).
+ *   d_transcript DEVICE pointer, receives 7*s+1 words: 2s x (G0,G1,G2), then q[0..s]
+ *                (a VC_SUM layer 0: 2*s words, s x (G0,G1); vc_transcript_words gives the count for any layer).
+ *   cap_words    capacity of d_transcript in words (VC_ERR_ARG if < vc_transcript_words(c, layer)).
  * Must be called with layer = 0,1,...,d-1 in order after vc_evaluate, with the same seed
  * (else VC_ERR_STATE).  Leaves (z, claim, counter) on the device for the next call. */
 int vc_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_transcript, uint64_t cap_words,

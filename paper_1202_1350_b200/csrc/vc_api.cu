@@ -11,6 +11,7 @@
 #include "vc_kernels.cuh"
 #include "vc_line.cuh"
 #include "vc_round.cuh"
+#include "vc_sum.cuh"
 
 namespace vc {
 std::atomic<uint64_t> g_launches{0};
@@ -131,22 +132,24 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
         if (!L.type || !L.in1 || !L.in2) return VC_ERR_ARG;
         const uint64_t n = 1ull << L.log_size, nb = 1ull << c->logs[i + 1];
         bool tree = true, self = true, onetype = true;
-        for (uint64_t g = 0; g < n; g++) {
+        if (i == 0 && L.log_size == 0 && L.type[0] == VC_SUM) c->sum_out = true;    // the one sum gate over all of layer 1: in1 / in2 are not read
+        for (uint64_t g = 0; g < n && !(i == 0 && c->sum_out); g++) {
             if (L.type[g] > 3 || L.in1[g] >= nb || L.in2[g] >= nb) return VC_ERR_SHAPE;
             tree = tree && L.in1[g] == 2 * g && L.in2[g] == 2 * g + 1;
             self = self && L.in1[g] == g && L.in2[g] == g;
             onetype = onetype && L.type[g] == L.type[0];
         }
         c->wiring[i] = !onetype ? 0u : (tree ? 1u : (self ? 2u : 0u));
+        if (i == 0 && c->sum_out) c->wiring[i] = 0u;
         const bool no_rule = getenv("VC_NO_WIRE_RULE") != nullptr;     // read at every load: records are read unless tree / self
-        if (c->wiring[i] == 0 && !no_rule && fit_wire_rule(L, c->logs[i + 1], c->wrule[i])) c->wiring[i] = 3u;
+        if (c->wiring[i] == 0 && !no_rule && !(i == 0 && c->sum_out) && fit_wire_rule(L, c->logs[i + 1], c->wrule[i])) c->wiring[i] = 3u;
         c->h_type[i].assign(L.type, L.type + n);
         c->h_in1[i].assign(L.in1, L.in1 + n);
         c->h_in2[i].assign(L.in2, L.in2 + n);
         max_gates = std::max(max_gates, n);
         max_tab = std::max(max_tab, nb);
         const uint32_t s = c->logs[i + 1];
-        total += 7ull * s + 1;
+        total += c->layer_words(i);
         const uint32_t used = std::min<uint32_t>(s, vc::LINE_NT + vc::LINE_TB);
         part = std::max(part, (size_t)(1ull << (s - used)) * (s > 1 ? s - 1 : 1));
     }
@@ -205,19 +208,49 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     const uint64_t n_in = 1ull << c->log_input;
     CUDA_TRY(cudaMemsetAsync(&c->d_state->flags, 0, sizeof(unsigned int), st));   // the status word reports THIS evaluation
     if (c->schedule != 1) {                      // one cooperative launch for the whole evaluation when the circuit allows it
-        const int rc = vc::enqueue_eval_fused(c, d_input, d_outputs, st);
+        int rc = vc::enqueue_eval_fused(c, d_input, d_outputs, st);
+        if (rc == VC_OK && c->sum_out) rc = vc::enqueue_sum_eval(c, d_outputs, st);
         if (rc == VC_OK) { c->next_layer = 0; return VC_OK; }
         if (rc != VC_ERR_STATE) return rc;
     }
     VC_LAUNCH(VC_K_EVAL, vc::k_copy_input, grid_for(n_in, c->sm_count), vc::RED_BLOCK, 0, st, d_input, c->d_V[d], n_in, c->d_state);
-    for (int i = (int)d - 1; i >= 0; i--) {
+    for (int i = (int)d - 1; i >= (int)c->first_pair_layer(); i--) {
         const uint32_t n = 1u << c->logs[i];
         VC_LAUNCH(VC_K_EVAL, vc::k_eval, grid_for(n, c->sm_count, 2), vc::RED_BLOCK, 0, st, c->d_type[i], c->d_in1[i], c->d_in2[i],
                   c->d_V[i + 1], c->d_V[i], (i == 0 ? d_outputs : (uint64_t *)nullptr), n);
     }
     CUDA_TRY(cudaGetLastError());
+    if (c->sum_out) { const int rc = vc::enqueue_sum_eval(c, d_outputs, st); if (rc != VC_OK) return rc; }
     c->next_layer = 0;
     return VC_OK;
+}
+
+// ------------------------------------------------------------------ the sum gate of large fan-in at the output (vc_sum.cuh)
+int vc::enqueue_sum_eval(vc_circuit *c, uint64_t *d_outputs, cudaStream_t st) {
+    const uint64_t n = 1ull << c->logs[1];
+    if (cudaMemsetAsync(&c->d_state->ticket, 0, sizeof(unsigned int), st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    VC_LAUNCH(VC_K_EVAL, vc::k_sum_eval, grid_for(n, c->sm_count), vc::RED_BLOCK, 0, st, c->d_V[1], n, c->d_V[0], d_outputs, c->d_part, c->d_state);
+    return cudaGetLastError() == cudaSuccess ? VC_OK : VC_ERR_CUDA;
+}
+
+// layer 0 of a sum-gate circuit: s rounds, one pass over the folded table per round (the fold of round j and the sums of
+// round j+1 share it), the last rounds in one CTA; leaves z = r, claim = V~_1(r), ctr = s for layer 1
+int vc::enqueue_sum_layer(vc_circuit *c, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {
+    const uint32_t s = c->logs[1];
+    const uint64_t n = 1ull << s;
+    vc::DevState *S = c->d_state;
+    if (cudaMemsetAsync(&S->ticket, 0, sizeof(unsigned int), st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    VC_LAUNCH(VC_K_ROUND, vc::k_sum_first, grid_for(n / 2, c->sm_count), vc::RED_BLOCK, 0, st, c->d_V[1], n, seed, c->d_part, S, d_tr);
+    const uint64_t *tab = c->d_V[1];
+    uint32_t j = 0;
+    for (; s - j > vc::SUM_TAIL_LOG; j++) {              // tab holds 2^(s-j) words, message j is out, r_j is drawn
+        uint64_t *out = (j & 1) ? c->d_T1 : c->d_T0;
+        const uint64_t half = n >> (j + 1);
+        VC_LAUNCH(VC_K_ROUND, vc::k_sum_fold, grid_for(half / 2, c->sm_count), vc::RED_BLOCK, 0, st, tab, out, half, j, c->d_part, S, d_tr);
+        tab = out;
+    }
+    VC_LAUNCH(VC_K_ROUND, vc::k_sum_tail, 1, vc::SUM_TAIL_T, 0, st, tab, s - j, j, S, d_tr);
+    return cudaGetLastError() == cudaSuccess ? VC_OK : VC_ERR_CUDA;
 }
 
 // ------------------------------------------------------------------ a2-a7, streaming schedule
@@ -262,10 +295,11 @@ extern "C" int vc_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint
     if (layer >= c->d) return VC_ERR_ARG;
     if (c->next_layer < 0 || (uint32_t)c->next_layer != layer) return VC_ERR_STATE;
     if (layer > 0 && seed != c->seed) return VC_ERR_STATE;
-    if (cap_words < 7ull * c->logs[layer + 1] + 1) return VC_ERR_ARG;
+    if (cap_words < c->layer_words(layer)) return VC_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc;
-    if (c->schedule != 1 && vc::fused_supported(c, layer)) rc = vc::enqueue_layer_fused(c, layer, seed, d_transcript, st);
+    if (layer == 0 && c->sum_out) rc = vc::enqueue_sum_layer(c, seed, d_transcript, st);
+    else if (c->schedule != 1 && vc::fused_supported(c, layer)) rc = vc::enqueue_layer_fused(c, layer, seed, d_transcript, st);
     else rc = vc::enqueue_layer_streaming(c, layer, seed, d_transcript, st);
     if (rc != VC_OK) return rc;
     c->seed = seed;
@@ -278,7 +312,10 @@ extern "C" int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, ui
     if (cap_words < c->total_words) return VC_ERR_ARG;
     if (c->next_layer != 0) return VC_ERR_STATE;
     if (c->schedule != 1 && vc::fused_supported(c, 0)) {     // whole proof in one cooperative launch
-        int rc = vc::enqueue_layers_fused(c, 0, c->d, seed, d_transcript, (cudaStream_t)cuda_stream);
+        int rc = VC_OK;
+        if (c->sum_out) rc = vc::enqueue_sum_layer(c, seed, d_transcript, (cudaStream_t)cuda_stream);   // then the fan-in-two layers 1 .. d-1
+        if (rc == VC_OK && c->first_pair_layer() < c->d)
+            rc = vc::enqueue_layers_fused(c, c->first_pair_layer(), c->d, seed, d_transcript + (c->sum_out ? c->layer_words(0) : 0), (cudaStream_t)cuda_stream);
         if (rc != VC_OK) return rc;
         c->seed = seed;
         c->next_layer = (int)c->d;
@@ -286,7 +323,7 @@ extern "C" int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, ui
     }
     uint64_t w = 0;
     for (uint32_t i = 0; i < c->d; i++) {
-        const uint64_t nw = 7ull * c->logs[i + 1] + 1;
+        const uint64_t nw = c->layer_words(i);
         int rc = vc_prove_layer(c, i, seed, d_transcript + w, nw, cuda_stream);
         if (rc != VC_OK) return rc;
         w += nw;
@@ -315,7 +352,7 @@ extern "C" int vc_run_host(vc_circuit *c, const uint64_t *h_input, uint64_t seed
 
 // ------------------------------------------------------------------ sizes, debug, probes
 extern "C" uint64_t vc_transcript_words(const vc_circuit *c, uint32_t layer) {
-    return (c && layer < c->d) ? 7ull * c->logs[layer + 1] + 1 : 0;
+    return (c && layer < c->d) ? c->layer_words(layer) : 0;
 }
 extern "C" uint64_t vc_total_transcript_words(const vc_circuit *c) { return c ? c->total_words : 0; }
 extern "C" uint32_t vc_depth(const vc_circuit *c) { return c ? c->d : 0; }

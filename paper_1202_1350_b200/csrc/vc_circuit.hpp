@@ -39,7 +39,12 @@ struct vc_circuit {
     int sm_count = 148;
     int coop_ok = 0;
 
+    bool sum_out = false;                       // layer 0 is the single VC_SUM gate over all of layer 1
+
     uint32_t log_below(uint32_t i) const { return logs[i + 1]; }
+    // transcript words of layer i: 2s x (G0,G1,G2) then q[0..s]; the sum gate: s x (G0,G1)
+    uint64_t layer_words(uint32_t i) const { return (sum_out && i == 0) ? 2ull * logs[1] : 7ull * logs[i + 1] + 1; }
+    uint32_t first_pair_layer() const { return sum_out ? 1u : 0u; }   // first layer proved by the fan-in-two engines
 };
 
 namespace vc {
@@ -49,6 +54,8 @@ struct ProfRec { int kind; cudaEvent_t a, b; };
 extern bool g_profile;                      // vc_profile_enable: CUDA events around every launch, by kind
 void prof_push(int kind, cudaEvent_t a, cudaEvent_t b);
 int enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
+int enqueue_sum_layer(vc_circuit *c, uint64_t seed, uint64_t *d_tr, cudaStream_t st);                  // vc_api.cu (vc_sum.cuh)
+int enqueue_sum_eval(vc_circuit *c, uint64_t *d_outputs, cudaStream_t st);
 int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);  // vc_fused.cu
 int fused_supported(const vc_circuit *c, uint32_t layer);
 int fused_init(vc_circuit *c);

@@ -109,8 +109,9 @@ __device__ __forceinline__ void eval_grid_barrier(unsigned long long *cnt, uint3
     }
     __syncthreads();
 }
+// top: the first layer evaluated here is d-1, the last is `top` (0; 1 when layer 0 is the sum gate, which has its own kernel)
 __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint32_t d, const uint64_t *in, uint64_t *out0,
-                                                          DevState *st, unsigned long long *cnt) {
+                                                          DevState *st, unsigned long long *cnt, int top) {
     const uint32_t tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
     uint32_t gen = 0;
     {
@@ -126,7 +127,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
     }
     extern __shared__ __align__(16) uint64_t ev_sm[];   // the narrow tail: two value tables of 2^(EVAL_NARROW_LOG+1) words
     int i = (int)d - 1;
-    for (; i >= 0; i--) {                         // grid-wide layers, separated by a counter rendezvous
+    for (; i >= top; i--) {                       // grid-wide layers, separated by a counter rendezvous
         if (L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1) break;
         const uint32_t n = 1u << L[i].log_n;
         const Wires wr(L[i]);
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
             if (i == 0 && out0) out0[g] = v;
         }
     }
-    if (i < 0) return;
+    if (i < top) return;
     // ---- CTA 0 finishes the narrow layers alone: values ping-pong in shared memory (every V_i is still written out
     // for the prover), and the records of the next layer are fetched before the barrier that ends the current one
     eval_grid_barrier(cnt, gen);
@@ -163,7 +164,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
     };
     fetch(i);
     __syncthreads();
-    for (; i >= 0; i--) {
+    for (; i >= top; i--) {
         const uint32_t n = 1u << L[i].log_n;
         uint64_t *Vo = const_cast<uint64_t *>(L[i].V);
 #pragma unroll
@@ -175,7 +176,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
                 if (i == 0 && out0) out0[g] = v;
             }
         }
-        if (i > 0) fetch(i - 1);
+        if (i > top) fetch(i - 1);
         __syncthreads();
         uint64_t *t = cur; cur = nxt; nxt = t;
     }
@@ -434,7 +435,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         lp.wiring = i < c->d ? c->wiring[i] : W_GENERIC;
         if (i < c->d) lp.rule = c->wrule[i];
         lp.type0 = i < c->d ? c->h_type[i][0] : 0;
-        if (i < c->d) {
+        if (i < c->d && !(i == 0 && c->sum_out)) {       // the sum gate is not a fan-in-two layer: vc_sum.cuh proves it
             std::vector<CtaPlan> cta;
             plan_layer(c, i, fh.grid, lp, cta, smem_need);
             if (lp.kind == 1) { cta_off[i] = all_cta.size(); all_cta.insert(all_cta.end(), cta.begin(), cta.end()); }
@@ -469,7 +470,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         bool ok = cudaFuncSetAttribute(k_eval_all, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EVAL_SMEM) == cudaSuccess &&
                   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&eper, k_eval_all, EVAL_T, EVAL_SMEM) == cudaSuccess && eper >= 1;
         bool seen_narrow = false;
-        for (int i = (int)c->d - 1; i >= 0 && ok; i--) {
+        for (int i = (int)c->d - 1; i >= (int)c->first_pair_layer() && ok; i--) {
             const bool narrow = c->logs[i] <= EVAL_NARROW_LOG && c->logs[i + 1] <= EVAL_NARROW_LOG + 1;
             if (seen_narrow && !narrow) ok = false;
             seen_narrow = seen_narrow || narrow;
@@ -480,6 +481,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     fh.group.resize(c->d);
     for (uint32_t i = 0; i < c->d; i++) fh.group[i] = h[i].kind == 0 ? 1 : (h[i].thin ? 2 : 4);
+    if (c->sum_out) fh.group[0] = 0;
     if (const char *e = getenv("VC_SINGLE_KERNEL")) fh.single_kernel = e[0] == '1';
     {   // the cluster engine takes every layer it can plan (VC_NO_CLUSTER=1: never, for A/B measurements)
         const char *nc = getenv("VC_NO_CLUSTER");
@@ -505,7 +507,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         (void)cudaGetLastError();
         bool any = false;
         if (csize) {
-            for (uint32_t i = 0; i < c->d; i++) {
+            for (uint32_t i = c->first_pair_layer(); i < c->d; i++) {
                 size_t need = dyn;
                 if (plan_cluster_layer(c, i, csize, hc[i], need) && fixed + need <= F_SMEM_MAX) { dyn = need; fh.group[i] = 8; any = true; }
                 else hc[i] = ClLayer{};
@@ -540,7 +542,7 @@ int fused_supported(const vc_circuit *c, uint32_t) { return find(c) != nullptr; 
 // proves layers [begin, end) in ONE cooperative launch
 int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t seed, uint64_t *d_tr, cudaStream_t st) {
     FusedHost *fh = find(c);
-    if (!fh) return VC_ERR_STATE;
+    if (!fh || begin < c->first_pair_layer()) return VC_ERR_STATE;
     // runs of layers by kernel group: {narrow, thin} -> k_fused<3>, {wide} -> k_fused<4>; more than F_MAX_RUNS runs -> one k_fused<7>
     std::vector<std::pair<uint32_t, int>> runs;          // (first layer, mask)
     for (uint32_t i = begin; i < end; i++) {
@@ -553,7 +555,7 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         if (!has_cl) { runs.clear(); runs.emplace_back(begin, 7); }
         else for (auto &r : runs) if (r.second != 8) r.second = 7;
     }
-    if (begin == 0) {   // a proof starts: the rendezvous slots and their epoch start clean whatever an earlier, aborted launch left behind
+    if (begin == c->first_pair_layer()) {   // a proof starts: the rendezvous slots and their epoch start clean whatever an earlier, aborted launch left behind
         if (cudaMemsetAsync(fh->d_slots, 0, (size_t)F_RING * F_SLOT_WORDS * 8, st) != cudaSuccess ||
             cudaMemsetAsync(&c->d_state->bar_gen, 0, sizeof(unsigned int), st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
     }
@@ -583,7 +585,7 @@ int enqueue_layers_fused(vc_circuit *c, uint32_t begin, uint32_t end, uint64_t s
         }
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
-        for (uint32_t i = b0; i < e0; i++) off += 7ull * c->logs[i + 1] + 1;
+        for (uint32_t i = b0; i < e0; i++) off += c->layer_words(i);
     }
     return VC_OK;
 }
@@ -593,7 +595,7 @@ int fused_layer_kinds(const vc_circuit *c, uint32_t *h_kind) {
     if (!fh) return VC_ERR_STATE;
     for (uint32_t i = 0; i < c->d; i++) {
         const int g = fh->group[i];
-        h_kind[i] = g == 8 ? VC_K_CLUSTER : g == 1 ? VC_K_FUSED_NARROW : g == 2 ? VC_K_FUSED_THIN : VC_K_FUSED_WIDE;
+        h_kind[i] = g == 0 ? VC_K_ROUND : g == 8 ? VC_K_CLUSTER : g == 1 ? VC_K_FUSED_NARROW : g == 2 ? VC_K_FUSED_THIN : VC_K_FUSED_WIDE;
     }
     return VC_OK;
 }
@@ -611,7 +613,8 @@ int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outpu
     if (!fh || !fh->eval_ok) return VC_ERR_STATE;
     if (cudaMemsetAsync(fh->d_evcnt, 0, 8, st) != cudaSuccess) return VC_ERR_CUDA;
     const LayerPlan *L = fh->d_plan; uint32_t d = c->d; DevState *S = c->d_state; unsigned long long *cnt = fh->d_evcnt;
-    void *params[] = {&L, &d, &d_input, &d_outputs, &S, &cnt};
+    int top = (int)c->first_pair_layer();
+    void *params[] = {&L, &d, &d_input, &d_outputs, &S, &cnt, &top};
     cudaEvent_t ea = nullptr, eb = nullptr;
     if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
     cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_eval_all, dim3(fh->grid), dim3(EVAL_T), params, EVAL_SMEM, st);

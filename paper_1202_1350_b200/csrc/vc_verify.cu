@@ -98,6 +98,14 @@ extern "C" int vc_verify_transcript(const vc_circuit *c, const uint64_t *h_input
         std::vector<u64> Tz, T1, T2;
         for (uint32_t i = 0; i < c->d; i++) {
             const uint32_t s = c->logs[i + 1];
+            if (i == 0 && c->sum_out) {          // the sum gate (VC_SUM in vc.h): s linear rounds, then the claim is V~_1(r) at z = r
+                for (uint32_t m = 0; m < s; m++, tr += 2) {
+                    if (fp61::add(tr[0], tr[1]) != claim) { *fail_layer = 0; *fail_round = m; return VC_OK; }
+                    z[m] = fp61::draw(seed, ctr++);
+                    claim = fp61::add(tr[0], fp61::mul(z[m], fp61::sub(tr[1], tr[0])));
+                }
+                continue;
+            }
             for (uint32_t m = 0; m < 2 * s; m++, tr += 3) {
                 if (fp61::add(tr[0], tr[1]) != claim) { *fail_layer = i; *fail_round = m; return VC_OK; }
                 r[m] = fp61::draw(seed, ctr++);

@@ -268,6 +268,10 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
     for (uint32_t i = 0; i < d; i++) {
         const uint32_t s = c->logs[i + 1];
         u64 *blk = h_pts + (size_t)i * 3 * MAX_VARS, *r1 = blk + MAX_VARS, *r2 = blk + 2 * MAX_VARS, *zn = blk + 3 * MAX_VARS;
+        if (i == 0 && c->sum_out) {              // the sum gate: s draws, and they ARE the next point (no r2, no tau)
+            for (uint32_t k = 0; k < s; k++) zn[k] = r1[k] = fp61::draw(seed, ctr++);
+            continue;
+        }
         for (uint32_t k = 0; k < s; k++) r1[k] = fp61::draw(seed, ctr++);
         for (uint32_t k = 0; k < s; k++) r2[k] = fp61::draw(seed, ctr++);
         taus[i] = fp61::draw(seed, ctr++);
@@ -279,7 +283,8 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
     auto blocks_for = [&](uint64_t n) { return (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((n + VT - 1) / VT, (uint64_t)vh->blocks)); };
     VC_LAUNCH(VC_K_MISC, k_v_mle, blocks_for(1ull << c->logs[0]), VT, V_TAB_WORDS * 8, st, d_outputs, c->logs[0], vh->d_pts, vh->d_part,
               vh->d_flags, vh->d_res, vh->d_flags + 1);
-    for (uint32_t i = 0; i < d; i++)
+    if (c->sum_out && cudaMemsetAsync(vh->d_res + 1, 0, 4 * 8, st) != cudaSuccess) return VC_ERR_CUDA;   // no wiring sums for the sum gate
+    for (uint32_t i = c->first_pair_layer(); i < d; i++)
         VC_LAUNCH(VC_K_MISC, k_v_wiring, blocks_for(1ull << c->logs[i]), VT, 3 * V_TAB_WORDS * 8, st, c->d_type[i], c->d_in1[i], c->d_in2[i],
                   c->logs[i], c->logs[i + 1], vh->d_pts + (size_t)i * 3 * MAX_VARS, vh->d_part, vh->d_flags, vh->d_res + 1 + 4 * (size_t)i);
     VC_LAUNCH(VC_K_MISC, k_v_mle, blocks_for(1ull << c->log_input), VT, V_TAB_WORDS * 8, st, d_input, c->log_input,
@@ -307,6 +312,13 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
     for (uint32_t i = 0; i < d; i++) {
         const uint32_t s = c->logs[i + 1];
         const u64 *blk = h_pts + (size_t)i * 3 * MAX_VARS;
+        if (i == 0 && c->sum_out) {
+            for (uint32_t m = 0; m < s; m++, tr += 2) {
+                if (fp61::add(tr[0], tr[1]) != claim) { *fail_layer = 0; *fail_round = m; return VC_OK; }
+                claim = fp61::add(tr[0], fp61::mul(blk[MAX_VARS + m], fp61::sub(tr[1], tr[0])));
+            }
+            continue;
+        }
         for (uint32_t m = 0; m < 2 * s; m++, tr += 3) {
             if (fp61::add(tr[0], tr[1]) != claim) { *fail_layer = i; *fail_round = m; return VC_OK; }
             claim = quad_at(tr, m < s ? blk[MAX_VARS + m] : blk[2 * MAX_VARS + (m - s)]);

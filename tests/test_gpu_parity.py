@@ -384,6 +384,61 @@ def test_matmul_equality_circuit_single_output_bit_exact(vc, log_m, wrong):
         gc.close()
 
 
+SUM_GATE_CASES = [
+    ("f2", 1), ("f2", 5), ("f2", 11), ("f2", 12), ("f2", 17),     # table = tail only; tail boundary (2^11) and one, six folds before it
+    ("f0", 4), ("f0", 13),                                       # 119 chain layers under the sum gate
+    ("alone", 9), ("alone", 14),                                  # d = 1: the sum gate reads the input directly, random F_p words
+]
+
+
+@pytest.mark.parametrize("kind,log_n", SUM_GATE_CASES)
+def test_sum_gate_of_large_fan_in_bit_exact(vc, kind, log_n):
+    """SURVEY.md §8f NEXT-4 / PAPER.md:220, :222 (reading c-19): the paper's own F2 and F0 circuits end in ONE sum gate
+    over all of layer 1 (VC_SUM).  Outputs, every transcript word and the final state against the oracle, on the fused and
+    the streaming schedule, whole proof and layer by layer; both verifiers accept; a flipped word of the sum gate's rounds
+    is rejected at its round by both."""
+    import torch
+    if kind == "alone":
+        rng = random.Random(log_n)
+        x = np.array([rng.randrange(P) for _ in range(1 << log_n)], dtype=np.uint64)
+        z0 = np.zeros(1, np.uint32)
+        c = W.Circuit([W.Layer(0, np.array([W.SUM], np.uint8), z0, z0)], log_n, x, "sum gate alone")
+    else:
+        c = (W.f2_sum_circuit if kind == "f2" else W.f0_sum_circuit)(log_n, 80 + log_n)
+    seed = 300 + log_n
+    oc = oracle.OracleCircuit(c)
+    want_out, want_tr, want_z, want_claim = oc.prove(c.input, seed)
+    for schedule, layerwise in ((0, False), (1, False), (0, True)):
+        gc, out, tr = _gpu_prove(vc, c, seed, schedule=schedule, layerwise=layerwise)
+        assert gc.words == want_tr.size == c.total_transcript_words
+        assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (kind, log_n, schedule, layerwise)
+        z, claim, ctr = gc.state()[:3]
+        assert claim == want_claim and np.array_equal(z[:c.log_input], want_z[:c.log_input])
+        assert gc.verify(c.input, out, seed, tr) == (True, 0, 0) and gc.verify_device(seed) == (True, 0, 0)
+        s = c.log_below(0)
+        for w in sorted({0, 2 * s - 1, s}):
+            bad = tr.copy(); bad[w] = (int(bad[w]) + 1) % P
+            want = oc.verify(c.input, out, seed, bad)
+            assert want == (False, 0, w // 2)
+            assert gc.verify(c.input, out, seed, bad) == want
+            assert gc.verify_device(seed, d_transcript=torch.from_numpy(bad.view(np.int64)).cuda()) == want
+        gc.close()
+
+
+def test_sum_gate_only_as_the_single_gate_of_layer_0(vc):
+    """VC_SUM anywhere else is a shape error at load (include/vc.h)."""
+    c = W.f2_sum_circuit(4, 1)
+    c.layers[1].type[3] = W.SUM
+    with pytest.raises(vc.VCError) as e:
+        vc.Circuit(c)
+    assert e.value.code == 2
+    c = W.f2_circuit(3, 1)
+    c.layers[1].type[:] = W.SUM            # a two-gate layer of SUM gates
+    with pytest.raises(vc.VCError) as e:
+        vc.Circuit(c)
+    assert e.value.code == 2
+
+
 def test_run_host_end_to_end_matches(vc):
     import torch
     c = W.config(1)
