@@ -52,6 +52,22 @@ typedef struct {
  * of range, unknown type, VC_SUM anywhere but as the single gate of layer 0), VC_ERR_CUDA / VC_ERR_NOMEM. */
 int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit **out);
 
+/* vc_circuit_load_hosted — the "copy-every-message approach" (§5.1.3, the paper's stated future work;
+ * SURVEY.md §8(f) NEXT-3) for layers whose gates do not fit device memory.  Same arguments and checks as vc_circuit_load, but
+ * the per-gate data — records (9 B per gate) and weights (8 B per gate) — stays in pinned HOST memory (the record arrays
+ * are copied once into the handle and page-locked there); the device holds the value tables, the fold tables and two chunk
+ * slots of 2^chunk_log gates (8 <= chunk_log <= 28, else VC_ERR_ARG).  For EVERY message of a layer the whole layer
+ * is streamed through the slots piece by piece: H2D of a piece's records and weights, the piece's contribution to the
+ * message (with the pending weight update of the previous challenge applied first), D2H of its updated weights, the
+ * copies of neighbouring pieces overlapping the kernel on two internal streams.  vc_evaluate streams the records once per
+ * layer.  Every other call (vc_prove_layer, vc_prove, vc_run_host, vc_verify_transcript, sizes) behaves as for a resident
+ * circuit and produces the same words; vc_set_schedule accepts only 2 for such a handle (and 2 only for such a handle),
+ * vc_verify_transcript_device returns VC_ERR_STATE (its wiring sums need device-resident records). */
+int vc_circuit_load_hosted(const vc_layer *layers, uint32_t d, uint32_t log_input, uint32_t chunk_log, vc_circuit **out);
+/* bytes a hosted circuit moved over the host link in its last vc_evaluate (h2d only) or since layer 0 of its last proof;
+ * VC_ERR_STATE for a resident circuit */
+int vc_debug_hosted_bytes(const vc_circuit *c, uint64_t *h2d, uint64_t *d2h);
+
 /* vc_evaluate — layered circuit evaluation (step a1; §6.2.4):
  * V_d = input; for i = d-1..0: V_i[g] = f_type(V_{i+1}[in1[g]], V_{i+1}[in2[g]])  (a VC_SUM output: the sum of V_1).
  *   d_input   DEVICE pointer, 2^log_input canonical words (read).  A word >= p is detected ON THE DEVICE while the input
@@ -145,7 +161,8 @@ int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind);
 int vc_debug_layer_wiring(const vc_circuit *c, uint32_t *h_mode);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */
 uint64_t vc_launch_count(void);
-/* selects the kernel schedule: 0 = auto (default), see DESIGN.md "Schedules" for the others */
+/* selects the kernel schedule: 0 = auto (default), 1 = streaming (one kernel per protocol step); 2 = copy-every-message, the
+ * fixed schedule of a vc_circuit_load_hosted handle (VC_ERR_STATE for any other combination) */
 int vc_set_schedule(vc_circuit *c, int schedule);
 
 /* Field/PRNG probes for the GPU unit tests: out[i] = op(a[i], b[i]) on the device, n words each,

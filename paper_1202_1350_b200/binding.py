@@ -16,7 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
-    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring", "vc_circuit_load_hosted", "vc_debug_hosted_bytes",
 ]
 
 
@@ -72,6 +72,8 @@ def lib():
             "vc_debug_trace": (i32, [vp, vp, u32, vp]),
             "vc_debug_layer_kinds": (i32, [vp, vp]),
             "vc_debug_layer_wiring": (i32, [vp, vp]),
+            "vc_circuit_load_hosted": (i32, [vp, u32, u32, u32, vp]),
+            "vc_debug_hosted_bytes": (i32, [vp, vp, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
         }
@@ -115,8 +117,9 @@ def _host_ptr(a) -> int:
 
 
 # ---------------------------------------------------------------------------- flat C-ABI mirrors
-def vc_circuit_load(layers, log_input: int) -> int:
-    """layers: sequence of objects with log_size/type/in1/in2 (numpy, host), output layer first. Returns the handle."""
+def vc_circuit_load(layers, log_input: int, hosted_chunk_log=None) -> int:
+    """layers: sequence of objects with log_size/type/in1/in2 (numpy, host), output layer first. Returns the handle.
+    hosted_chunk_log: vc_circuit_load_hosted with slots of 2^hosted_chunk_log gates (records and weights stay on the host)."""
     arr = (_Layer * len(layers))()
     keep = []
     for i, L in enumerate(layers):
@@ -126,7 +129,10 @@ def vc_circuit_load(layers, log_input: int) -> int:
         keep += [t, a, b]
         arr[i] = _Layer(int(L.log_size), t.ctypes.data, a.ctypes.data, b.ctypes.data)
     h = C.c_void_p(0)
-    _check(lib().vc_circuit_load(arr, len(layers), int(log_input), C.byref(h)), "vc_circuit_load")
+    if hosted_chunk_log is None:
+        _check(lib().vc_circuit_load(arr, len(layers), int(log_input), C.byref(h)), "vc_circuit_load")
+    else:
+        _check(lib().vc_circuit_load_hosted(arr, len(layers), int(log_input), int(hosted_chunk_log), C.byref(h)), "vc_circuit_load_hosted")
     return h.value
 
 
@@ -190,10 +196,10 @@ def vc_total_transcript_words(handle: int) -> int:
 class Circuit:
     """Owns a vc_circuit handle plus the torch device buffers a proof needs (input, outputs, transcript)."""
 
-    def __init__(self, circuit):
+    def __init__(self, circuit, hosted_chunk_log=None):
         import torch
         self.torch = torch
-        self.handle = vc_circuit_load(circuit.layers, circuit.log_input)
+        self.handle = vc_circuit_load(circuit.layers, circuit.log_input, hosted_chunk_log)
         self.d = len(circuit.layers)
         self.log_input = circuit.log_input
         self.n_out = 1 << circuit.layers[0].log_size
@@ -256,6 +262,12 @@ class Circuit:
         h = np.zeros(self.d, dtype=np.uint32)
         _check(lib().vc_debug_layer_wiring(self.handle, h.ctypes.data), "vc_debug_layer_wiring")
         return h
+
+    def hosted_bytes(self):
+        """(h2d, d2h) bytes a hosted circuit moved in its last evaluation / proof (vc_debug_hosted_bytes)."""
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        _check(lib().vc_debug_hosted_bytes(self.handle, C.byref(a), C.byref(b)), "vc_debug_hosted_bytes")
+        return int(a.value), int(b.value)
 
     def flags(self) -> int:
         f = C.c_uint32(0)

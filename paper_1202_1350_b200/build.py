@@ -8,7 +8,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 SO = HERE / "libvc.so"
-SOURCES = ["vc_api.cu", "vc_fused.cu", "vc_verify.cu", "vc_verify_gpu.cu"]
+SOURCES = ["vc_api.cu", "vc_fused.cu", "vc_hosted.cu", "vc_verify.cu", "vc_verify_gpu.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

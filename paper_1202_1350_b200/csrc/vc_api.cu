@@ -60,6 +60,7 @@ extern "C" void vc_circuit_free(vc_circuit *c) {
     if (!c) return;
     vc::fused_free(c);
     vc::verifier_free(c);
+    vc::hosted_free(c);
     for (auto p : c->d_type) cudaFree(p);
     for (auto p : c->d_in1) cudaFree(p);
     for (auto p : c->d_in2) cudaFree(p);
@@ -157,7 +158,7 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
     c->part_words = part;
     c->d_type.assign(d, nullptr); c->d_in1.assign(d, nullptr); c->d_in2.assign(d, nullptr);
     c->d_V.assign(d + 1, nullptr);
-    for (uint32_t i = 0; i < d; i++) {
+    for (uint32_t i = 0; i < d && !c->hosted; i++) {     // hosted: the records never live on the device as a whole (vc_hosted.cu)
         const size_t n = (size_t)1 << c->logs[i];
         CUDA_TRY(cudaMalloc(&c->d_type[i], n));
         CUDA_TRY(cudaMalloc(&c->d_in1[i], n * 4));
@@ -167,7 +168,7 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
         CUDA_TRY(cudaMemcpy(c->d_in2[i], layers[i].in2, n * 4, cudaMemcpyHostToDevice));
     }
     for (uint32_t i = 0; i <= d; i++) CUDA_TRY(cudaMalloc(&c->d_V[i], (size_t)8 << c->logs[i]));
-    CUDA_TRY(cudaMalloc(&c->d_P, max_gates * 8));
+    if (!c->hosted) CUDA_TRY(cudaMalloc(&c->d_P, max_gates * 8));     // hosted: the weights live in pinned host memory
     CUDA_TRY(cudaMalloc(&c->d_T0, std::max<uint64_t>(max_tab / 2, 2) * 8));
     CUDA_TRY(cudaMalloc(&c->d_T1, std::max<uint64_t>(max_tab / 4, 2) * 8));
     CUDA_TRY(cudaMalloc(&c->d_part, part * 8));
@@ -185,14 +186,30 @@ static int load_impl(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_
     delete hs;
     CUDA_TRY(e);
     CUDA_TRY(cudaFuncSetAttribute(vc::k_line, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    if (c->hosted) { c->schedule = 2; return vc::hosted_init(c); }
     return vc::fused_init(c);
 }
 
+static int load_any(const vc_layer *layers, uint32_t d, uint32_t log_input, bool hosted, uint32_t chunk_log, vc_circuit **out);
 extern "C" int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_circuit **out) {
+    return load_any(layers, d, log_input, false, 0, out);
+}
+extern "C" int vc_circuit_load_hosted(const vc_layer *layers, uint32_t d, uint32_t log_input, uint32_t chunk_log, vc_circuit **out) {
+    if (chunk_log < 8 || chunk_log > 28) return VC_ERR_ARG;
+    return load_any(layers, d, log_input, true, chunk_log, out);
+}
+extern "C" int vc_debug_hosted_bytes(const vc_circuit *c, uint64_t *h2d, uint64_t *d2h) {
+    if (!c || !h2d || !d2h) return VC_ERR_ARG;
+    if (!c->hosted) return VC_ERR_STATE;
+    *h2d = c->h2d_bytes; *d2h = c->d2h_bytes;
+    return VC_OK;
+}
+static int load_any(const vc_layer *layers, uint32_t d, uint32_t log_input, bool hosted, uint32_t chunk_log, vc_circuit **out) {
     if (!layers || !out || d == 0) return VC_ERR_ARG;
     *out = nullptr;
     vc_circuit *c = new (std::nothrow) vc_circuit();
     if (!c) return VC_ERR_NOMEM;
+    c->hosted = hosted; c->chunk_log = chunk_log;
     int rc;
     try { rc = load_impl(layers, d, log_input, c); } catch (const std::bad_alloc &) { rc = VC_ERR_NOMEM; }
     if (rc != VC_OK) { vc_circuit_free(c); return rc; }
@@ -207,6 +224,11 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     const uint32_t d = c->d;
     const uint64_t n_in = 1ull << c->log_input;
     CUDA_TRY(cudaMemsetAsync(&c->d_state->flags, 0, sizeof(unsigned int), st));   // the status word reports THIS evaluation
+    if (c->hosted) {
+        const int rc = vc::hosted_evaluate(c, d_input, d_outputs, st);
+        if (rc == VC_OK) c->next_layer = 0;
+        return rc;
+    }
     if (c->schedule != 1) {                      // one cooperative launch for the whole evaluation when the circuit allows it
         int rc = vc::enqueue_eval_fused(c, d_input, d_outputs, st);
         if (rc == VC_OK && c->sum_out) rc = vc::enqueue_sum_eval(c, d_outputs, st);
@@ -298,7 +320,8 @@ extern "C" int vc_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint
     if (cap_words < c->layer_words(layer)) return VC_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc;
-    if (layer == 0 && c->sum_out) rc = vc::enqueue_sum_layer(c, seed, d_transcript, st);
+    if (c->hosted) rc = vc::hosted_prove_layer(c, layer, seed, d_transcript, st);
+    else if (layer == 0 && c->sum_out) rc = vc::enqueue_sum_layer(c, seed, d_transcript, st);
     else if (c->schedule != 1 && vc::fused_supported(c, layer)) rc = vc::enqueue_layer_fused(c, layer, seed, d_transcript, st);
     else rc = vc::enqueue_layer_streaming(c, layer, seed, d_transcript, st);
     if (rc != VC_OK) return rc;
@@ -311,7 +334,7 @@ extern "C" int vc_prove(vc_circuit *c, uint64_t seed, uint64_t *d_transcript, ui
     if (!c || !d_transcript) return VC_ERR_ARG;
     if (cap_words < c->total_words) return VC_ERR_ARG;
     if (c->next_layer != 0) return VC_ERR_STATE;
-    if (c->schedule != 1 && vc::fused_supported(c, 0)) {     // whole proof in one cooperative launch
+    if (!c->hosted && c->schedule != 1 && vc::fused_supported(c, 0)) {     // whole proof in one cooperative launch
         int rc = VC_OK;
         if (c->sum_out) rc = vc::enqueue_sum_layer(c, seed, d_transcript, (cudaStream_t)cuda_stream);   // then the fan-in-two layers 1 .. d-1
         if (rc == VC_OK && c->first_pair_layer() < c->d)
@@ -360,7 +383,8 @@ extern "C" uint32_t vc_log_size(const vc_circuit *c, uint32_t layer) { return (c
 extern "C" uint64_t vc_launch_count(void) { return vc::g_launches.load(); }
 
 extern "C" int vc_set_schedule(vc_circuit *c, int schedule) {
-    if (!c || schedule < 0 || schedule > 1) return VC_ERR_ARG;
+    if (!c || schedule < 0 || schedule > 2) return VC_ERR_ARG;
+    if ((schedule == 2) != c->hosted) return VC_ERR_STATE;      // schedule 2 is the one schedule of a hosted circuit, and only of it
     c->schedule = schedule;
     return VC_OK;
 }

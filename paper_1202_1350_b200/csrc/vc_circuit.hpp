@@ -39,6 +39,18 @@ struct vc_circuit {
     int sm_count = 148;
     int coop_ok = 0;
 
+    // hosted circuits (vc_circuit_load_hosted; vc_hosted.cu): records and weights stay in pinned host memory and are streamed
+    // through two device slots for every message (the copy-every-message approach)
+    bool hosted = false;
+    uint32_t chunk_log = 0;
+    std::vector<void *> pinned_ptrs;            // record arrays registered with cudaHostRegister
+    uint64_t *p_P = nullptr;                    // pinned host weights, max layer size
+    struct HostedSlot { uint8_t *type; uint32_t *in1, *in2; uint64_t *P; cudaEvent_t ready, done, back; };
+    HostedSlot slot[2] = {};
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_round = nullptr;
+    uint64_t *d_acc = nullptr;                  // running sums of a message across chunks (+ the start claim)
+    uint64_t h2d_bytes = 0, d2h_bytes = 0;      // moved by the last evaluation / proof of a hosted circuit
     bool sum_out = false;                       // layer 0 is the single VC_SUM gate over all of layer 1
 
     uint32_t log_below(uint32_t i) const { return logs[i + 1]; }
@@ -56,6 +68,10 @@ void prof_push(int kind, cudaEvent_t a, cudaEvent_t b);
 int enqueue_layer_streaming(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
 int enqueue_sum_layer(vc_circuit *c, uint64_t seed, uint64_t *d_tr, cudaStream_t st);                  // vc_api.cu (vc_sum.cuh)
 int enqueue_sum_eval(vc_circuit *c, uint64_t *d_outputs, cudaStream_t st);
+int hosted_init(vc_circuit *c);                                                                       // vc_hosted.cu
+void hosted_free(vc_circuit *c);
+int hosted_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, cudaStream_t st);
+int hosted_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);
 int enqueue_layer_fused(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d_tr, cudaStream_t st);  // vc_fused.cu
 int fused_supported(const vc_circuit *c, uint32_t layer);
 int fused_init(vc_circuit *c);

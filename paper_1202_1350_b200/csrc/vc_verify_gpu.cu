@@ -250,6 +250,7 @@ extern "C" int vc_verify_transcript_device(const vc_circuit *c, const uint64_t *
     if (!c || !d_input || !d_outputs || !d_transcript || !accept || !fail_layer || !fail_round) return VC_ERR_ARG;
     *accept = 0; *fail_layer = 0; *fail_round = 0;
     if (n_words != c->total_words) return VC_ERR_ARG;
+    if (c->hosted) return VC_ERR_STATE;                        // the wiring sums read device-resident records; a hosted circuit has none
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
     VerifierHost *vh = verifier_of(c);
