@@ -211,7 +211,9 @@ def run_ours(args):
     c.input = replicas.replica_input(c.input, W.data_seed(k or 2), rank)   # replicas: same circuit, another seeded input
     seed = W.challenge_seed(k or 2)
     L = vc.lib()
-    gc = vc.Circuit(c)
+    gc = vc.Circuit(c, hosted_chunk_log=args.hosted_chunk_log or None)
+    if args.hosted_chunk_log:
+        args.schedule = 2                        # the one schedule of a hosted handle (copy-every-message)
     gc.set_schedule(args.schedule)
     gc.set_input(c.input)
     stream = torch.cuda.current_stream()
@@ -410,6 +412,10 @@ def run_ours(args):
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(c.input.nbytes),
                         "d2h_bytes_per_step": int(8 * (gc.n_out + gc.words)), "ms_per_step": e2e_ms / args.steps},
                 "roofline": roofline, "cpu_baseline": cpu, "verifier": verifier}
+        if args.hosted_chunk_log:                # copy-every-message: the per-message traffic over the host link, inside the timed steps
+            hb = gc.hosted_bytes()
+            line["hosted"] = {"chunk_log": args.hosted_chunk_log, "proof_h2d_bytes": hb[0], "proof_d2h_bytes": hb[1],
+                              "note": "records and weights streamed from pinned host memory for every message (PAPER.md:165); counted on top of e2e's input/output copies"}
         print(json.dumps(line), flush=True)
     gc.close()
     if world > 1:
@@ -425,6 +431,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--hosted-chunk-log", type=int, default=0, help="time the copy-every-message approach (SURVEY.md §8f NEXT-3): records and weights in pinned host memory, streamed per message in pieces of 2^N gates")
     ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")
     ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | matmuleq:LOG_M (the single-output circuit of PAPER.md:230) | f2sum:N | f0sum:N (the paper's circuits with ONE sum gate of fan-in n at the output, PAPER.md:220) | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")

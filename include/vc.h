@@ -162,7 +162,7 @@ int vc_debug_layer_wiring(const vc_circuit *c, uint32_t *h_mode);
 /* number of kernels this library has launched since load (for bench.py's gpu_launches) */
 uint64_t vc_launch_count(void);
 /* selects the kernel schedule: 0 = auto (default), 1 = streaming (one kernel per protocol step); 2 = copy-every-message, the
- * fixed schedule of a vc_circuit_load_hosted handle (VC_ERR_STATE for any other combination) */
+ * fixed schedule of a vc_circuit_load_hosted handle (VC_ERR_STATE for any other combination); DESIGN.md §5 (schedules 0, 1) and §9e (schedule 2) */
 int vc_set_schedule(vc_circuit *c, int schedule);
 
 /* Field/PRNG probes for the GPU unit tests: out[i] = op(a[i], b[i]) on the device, n words each,
