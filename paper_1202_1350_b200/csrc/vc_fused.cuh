@@ -305,7 +305,15 @@ __device__ __forceinline__ void round_slot_to_transcript(const unsigned long lon
     const uint64_t hi = __shfl_down_sync(0xffffffffu, got, 1);
     if (lane >= 1 && lane < 7 && (lane & 1)) tr[(lane - 1) >> 1] = fp61::add(fp61::reduce62(got), fp61::mul(hi, 1ull << 32));
 }
-// warp 0, after the commit barrier: the rendezvous on the count word; the challenge is handed out afterwards
+// warp 0, after the commit barrier: the rendezvous on the count word; the challenge is handed out afterwards.
+// Memory-model note: the poll is ld.relaxed.gpu with no acquire fence behind it unless the round publishes data
+// (fence == true), although the recycling of slot epoch+2 is ordered through this rendezvous: the last CTA zero-stores the
+// slot, __threadfence()s, passes a CTA barrier, and only then its warp 0 arrives here with atom.relaxed; every other CTA
+// adds into that slot only after it has SEEN the full count.  Formally (PTX memory model) the observers would need an
+// acquire; on this hardware both the zero-store (made visible at L2 by the fence before the arrival) and the later red.add
+// are performed at the one L2 slice that owns the line, and the add is control-dependent on the poll, so it cannot be
+// performed before the count it waited for.  -DVC_RDV_ACQ puts a fence.acq_rel.gpu behind every poll (the formally
+// conforming variant): bit-identical results, +93 us per config-2 proof (1.294 -> 1.387 ms, 278 grid rounds) on the box.
 __device__ __forceinline__ void round_rendezvous(const FusedArgs &a, uint32_t ep, bool fence, uint64_t *rslot, uint64_t seed,
                                                  uint32_t ctr) {
     const uint64_t r = fp61::draw(seed, ctr);
@@ -315,7 +323,11 @@ __device__ __forceinline__ void round_rendezvous(const FusedArgs &a, uint32_t ep
         const uint64_t want = (uint64_t)gridDim.x;
         if ((atom_add(slot, F_CNT_ONE) >> 48) + 1 != want)
             while ((ld_relaxed(slot) >> 48) != want) { }
+#ifdef VC_RDV_ACQ
+        __threadfence();
+#else
         if (fence) __threadfence();
+#endif
         *rslot = r;
     }
 }
