@@ -72,26 +72,36 @@ def measured_peaks():
 
 # ---------------------------------------------------------------------------------------------- clocks
 class ClockSampler(threading.Thread):
+    """One `nvidia-smi --query-gpu=... -lms 20` process for the whole timed part (the recipe's clocks line in
+    B200_PROFILING.md), started before and killed after: forking a fresh nvidia-smi per sample re-initialises the driver
+    library every time, which delays the host's launches while it runs and showed up as +0.6 ms in the end-to-end leg."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
-        self.index, self.samples, self.stop_flag = index, [], threading.Event()
+        self.index, self.samples, self.stop_flag, self.proc = index, [], threading.Event(), None
 
     def run(self):
-        while not self.stop_flag.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
-                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.samples.append([p.strip() for p in out.split(",")])
-            except Exception:
-                pass
-            self.stop_flag.wait(0.1)
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index),
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) >= 6:
+                    self.samples.append(parts)
+                if self.stop_flag.is_set():
+                    break
+        except Exception:
+            pass
 
     def summary(self):
         self.stop_flag.set()
+        if self.proc is not None:
+            try:
+                self.proc.terminate()
+            except Exception:
+                pass
         self.join(timeout=6)
         sm = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
         mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
