@@ -223,7 +223,7 @@ extern "C" int vc_evaluate(vc_circuit *c, const uint64_t *d_input, uint64_t *d_o
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const uint32_t d = c->d;
     const uint64_t n_in = 1ull << c->log_input;
-    CUDA_TRY(cudaMemsetAsync(&c->d_state->flags, 0, sizeof(unsigned int), st));   // the status word reports THIS evaluation
+    CUDA_TRY(cudaMemsetAsync(&c->d_state->flags, 0, 2 * sizeof(unsigned int), st));   // the status word reports THIS evaluation; + k_eval_all's counter
     if (c->hosted) {
         const int rc = vc::hosted_evaluate(c, d_input, d_outputs, st);
         if (rc == VC_OK) c->next_layer = 0;

@@ -98,22 +98,65 @@ __global__ void __launch_bounds__(FT, 1) k_fused(FusedArgs a) {
 // values in shared memory and the next layer's records fetched ahead.
 constexpr int EVAL_T = 1024;
 constexpr uint32_t EVAL_NARROW_LOG = 11;
-__device__ __forceinline__ void eval_grid_barrier(unsigned long long *cnt, uint32_t &gen) {
+__device__ __forceinline__ void eval_grid_barrier(unsigned int *cnt, uint32_t &gen) {
     __syncthreads();
     if (threadIdx.x == 0) {
         gen++;
         __threadfence();
-        red_add(cnt, 1ull);
-        const unsigned long long want = (unsigned long long)gen * gridDim.x;
-        while (ld_acquire(cnt) < want) { }
+        asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
+        const unsigned int want = gen * gridDim.x;
+        unsigned int v;
+        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(cnt) : "memory"); } while (v < want);
     }
     __syncthreads();
 }
-// top: the first layer evaluated here is d-1, the last is `top` (0; 1 when layer 0 is the sum gate, which has its own kernel)
+// top: the first layer evaluated here is d-1, the last is `top` (0; 1 when layer 0 is the sum gate, which has its own kernel).
+// loc_bl > 0: layers d-1 .. loc_top have block-local wiring (tree: 2g, 2g+1; self: g, g; one gate type each), so a block of
+// 2^loc_bl inputs determines its own share of every one of them: a CTA checks and copies its inputs, then runs up the
+// layers in shared memory (every V_i is still written out for the prover) with block barriers only; the grid meets once,
+// after the local run, instead of once per layer.
+#ifndef VC_EVAL_LOC_LOG
+#define VC_EVAL_LOC_LOG 13
+#endif
+constexpr uint32_t EVAL_LOC_LOG = VC_EVAL_LOC_LOG;                   // inputs per block of the local run (two tables of 2^13 words: one wave of 128 blocks at n = 2^20)
 __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint32_t d, const uint64_t *in, uint64_t *out0,
-                                                          DevState *st, unsigned long long *cnt, int top) {
+                                                          DevState *st, int top, uint32_t loc_bl, int loc_top) {
+    unsigned int *cnt = &st->bar_count;              // zeroed together with the status word when vc_evaluate is enqueued
     const uint32_t tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
     uint32_t gen = 0;
+    extern __shared__ __align__(16) uint64_t ev_sm[];   // the narrow tail / the local run: two value tables of 2^(EVAL_NARROW_LOG+1) words
+    int i = (int)d - 1;
+    if (loc_bl) {
+        uint64_t *Vd = const_cast<uint64_t *>(L[d].V);
+        const uint32_t nblk = 1u << (L[d].log_n - loc_bl), B = 1u << loc_bl;
+        unsigned bad = 0;
+        for (uint32_t blk = b; blk < nblk; blk += G) {
+            uint64_t *cur = ev_sm, *nxt = ev_sm + B;
+            for (uint32_t u = tid; u < B; u += EVAL_T) {
+                const uint64_t w = in[(size_t)blk * B + u];
+                bad |= (w >= fp61::P);
+                Vd[(size_t)blk * B + u] = w;
+                cur[u] = w;
+            }
+            __syncthreads();
+            uint32_t share = B;                          // this block's entries of the layer below
+            for (int l = (int)d - 1; l >= loc_top; l--) {
+                const bool tree = L[l].wiring == W_TREE;
+                const uint32_t t0 = L[l].type0;
+                if (tree) share >>= 1;
+                uint64_t *Vo = const_cast<uint64_t *>(L[l].V) + (size_t)blk * share;
+                for (uint32_t g = tid; g < share; g += EVAL_T) {
+                    const uint64_t v = tree ? gate_f(t0, cur[2 * g], cur[2 * g + 1]) : gate_f(t0, cur[g], cur[g]);
+                    nxt[g] = v; Vo[g] = v;
+                    if (l == 0 && out0) out0[(size_t)blk * share + g] = v;
+                }
+                __syncthreads();
+                uint64_t *t = cur; cur = nxt; nxt = t;
+            }
+        }
+        if (bad) atomicOr(&st->flags, 1u);
+        i = loc_top - 1;
+    } else
     {
         uint64_t *Vd = const_cast<uint64_t *>(L[d].V);
         const uint64_t n = 1ull << L[d].log_n;
@@ -125,8 +168,6 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
         }
         if (bad) atomicOr(&st->flags, 1u);
     }
-    extern __shared__ __align__(16) uint64_t ev_sm[];   // the narrow tail: two value tables of 2^(EVAL_NARROW_LOG+1) words
-    int i = (int)d - 1;
     for (; i >= top; i--) {                       // grid-wide layers, separated by a counter rendezvous
         if (L[i].log_n <= EVAL_NARROW_LOG && L[i + 1].log_n <= EVAL_NARROW_LOG + 1) break;
         const uint32_t n = 1u << L[i].log_n;
@@ -182,7 +223,7 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
     }
 }
 
-constexpr size_t EVAL_SMEM = 2 * (size_t)(2u << EVAL_NARROW_LOG) * 8;
+constexpr size_t EVAL_SMEM = 2 * (size_t)((2u << EVAL_NARROW_LOG) > (1u << EVAL_LOC_LOG) ? (2u << EVAL_NARROW_LOG) : (1u << EVAL_LOC_LOG)) * 8;
 
 constexpr size_t F_SMEM_MAX = 227 * 1024;
 constexpr size_t F_MAX_RUNS = 8;                   // more runs of layer kinds than this: the all-kinds kernel, one launch
@@ -192,8 +233,9 @@ struct FusedHost {
     CtaPlan *d_cta = nullptr;
     unsigned long long *d_slots = nullptr;
     uint64_t *d_stamps = nullptr, *d_C = nullptr, *d_Tg = nullptr;
-    unsigned long long *d_evcnt = nullptr;
     bool eval_ok = false;
+    uint32_t eval_loc_bl = 0;                      // k_eval_all's block-local run: log2 inputs per block (0: none), last local layer
+    int eval_loc_top = 0;
     std::vector<int> group;                        // per layer: 1 narrow, 2 thin, 4 wide (which k_fused instantiation holds its code), 8 = the cluster engine
     int grid = 0;
     size_t smem = 0;
@@ -205,7 +247,7 @@ struct FusedHost {
 static std::vector<std::pair<const vc_circuit *, FusedHost *>> g_fused;   // heap entries: pointers handed out by find() stay valid
 static void release(FusedHost *f) {
     if (!f) return;
-    cudaFree(f->d_plan); cudaFree(f->d_cta); cudaFree(f->d_slots); cudaFree(f->d_stamps); cudaFree(f->d_C); cudaFree(f->d_Tg); cudaFree(f->d_evcnt); cudaFree(f->d_cl);
+    cudaFree(f->d_plan); cudaFree(f->d_cta); cudaFree(f->d_slots); cudaFree(f->d_stamps); cudaFree(f->d_C); cudaFree(f->d_Tg); cudaFree(f->d_cl);
     delete f;
 }
 
@@ -464,7 +506,6 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
     if (cudaMalloc(&fh.d_stamps, (size_t)(c->d + 1 + F_TRACE_WORDS) * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_C, max_gates * 8) != cudaSuccess) return VC_ERR_NOMEM;
     if (cudaMalloc(&fh.d_Tg, (size_t)(2u << F_TLOG) * 8) != cudaSuccess) return VC_ERR_NOMEM;
-    if (cudaMalloc(&fh.d_evcnt, 64) != cudaSuccess) return VC_ERR_NOMEM;
     {   // the one-launch evaluation needs: a co-resident grid, and narrow layers only at the output end
         int eper = 0;
         bool ok = cudaFuncSetAttribute(k_eval_all, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EVAL_SMEM) == cudaSuccess &&
@@ -477,6 +518,18 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         }
         (void)cudaGetLastError();
         fh.eval_ok = ok;
+        // the block-local run: layers d-1, d-2, ... while the wiring is tree (exactly half the layer below) or self (same size)
+        // and a block of 2^EVAL_LOC_LOG inputs still owns at least one gate; worth it from three layers on
+        if (ok && c->log_input > EVAL_LOC_LOG && !getenv("VC_NO_EVAL_LOCAL")) {
+            uint32_t share_log = EVAL_LOC_LOG;
+            int l = (int)c->d - 1;
+            for (; l >= (int)c->first_pair_layer(); l--) {
+                const uint32_t w = c->wiring[l];
+                if (w == 1 && c->logs[l] + 1 == c->logs[l + 1] && share_log > 0) share_log--;
+                else if (!(w == 2 && c->logs[l] == c->logs[l + 1])) break;
+            }
+            if ((int)c->d - 1 - l >= 3) { fh.eval_loc_bl = EVAL_LOC_LOG; fh.eval_loc_top = l + 1; }
+        }
     }
     for (uint32_t i = 0; i < c->d; i++) h[i].cta = cta_off[i] == (size_t)-1 ? nullptr : fh.d_cta + cta_off[i];
     fh.group.resize(c->d);
@@ -611,10 +664,10 @@ int fused_stamps(const vc_circuit *c, uint64_t *h, cudaStream_t st) {
 int enqueue_eval_fused(vc_circuit *c, const uint64_t *d_input, uint64_t *d_outputs, cudaStream_t st) {
     FusedHost *fh = find(c);
     if (!fh || !fh->eval_ok) return VC_ERR_STATE;
-    if (cudaMemsetAsync(fh->d_evcnt, 0, 8, st) != cudaSuccess) return VC_ERR_CUDA;
-    const LayerPlan *L = fh->d_plan; uint32_t d = c->d; DevState *S = c->d_state; unsigned long long *cnt = fh->d_evcnt;
-    int top = (int)c->first_pair_layer();
-    void *params[] = {&L, &d, &d_input, &d_outputs, &S, &cnt, &top};
+    const LayerPlan *L = fh->d_plan; uint32_t d = c->d; DevState *S = c->d_state;
+    int top = (int)c->first_pair_layer(), loc_top = fh->eval_loc_top;
+    uint32_t loc_bl = fh->eval_loc_bl;
+    void *params[] = {&L, &d, &d_input, &d_outputs, &S, &top, &loc_bl, &loc_top};
     cudaEvent_t ea = nullptr, eb = nullptr;
     if (g_profile) { cudaEventCreate(&ea); cudaEventCreate(&eb); cudaEventRecord(ea, st); }
     cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_eval_all, dim3(fh->grid), dim3(EVAL_T), params, EVAL_SMEM, st);

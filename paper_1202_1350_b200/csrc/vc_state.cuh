@@ -24,7 +24,7 @@ struct DevState {
     uint64_t G[4];             // last round's message (debug)
     unsigned int ticket;       // last-block-done counter of the streaming kernels
     unsigned int flags;        // bit 0: non-canonical input word seen
-    unsigned int bar_count;    // grid barrier of the cooperative layer kernel
+    unsigned int bar_count;    // rendezvous counter of k_eval_all (directly behind flags: one memset clears both)
     unsigned int bar_gen;
     uint64_t invfact[MAX_VARS + 1];  // 1/k! mod p, written once at load (Lagrange denominators)
 };

@@ -439,6 +439,34 @@ def test_sum_gate_only_as_the_single_gate_of_layer_0(vc):
     assert e.value.code == 2
 
 
+@pytest.mark.parametrize("log_n", [13, 14, 17])
+def test_block_local_evaluation_gives_every_layer_value(vc, monkeypatch, log_n):
+    """k_eval_all runs tree / self layers block by block in shared memory when the circuit starts with such layers (F2:
+    squares, then the add tree) and meets the grid once instead of once per layer: every V_i against the oracle, with the
+    local run and without it (VC_NO_EVAL_LOCAL=1 at load), also under a sum gate, also with a non-canonical input word."""
+    import torch
+    for c in (W.f2_circuit(log_n, 40 + log_n), W.f2_sum_circuit(log_n, 50 + log_n)):
+        V = oracle.OracleCircuit(c).evaluate(c.input)
+        for off in ("", "1"):
+            if off:
+                monkeypatch.setenv("VC_NO_EVAL_LOCAL", off)
+            else:
+                monkeypatch.delenv("VC_NO_EVAL_LOCAL", raising=False)
+            gc = vc.Circuit(c)
+            gc.set_input(c.input)
+            gc.evaluate()
+            assert gc.flags() == 0
+            for i in range(c.d + 1):
+                assert np.array_equal(gc.values(i), V[i]), (c.name, off, i)
+            assert np.array_equal(gc.outputs(), V[0])
+            bad = c.input.copy(); bad[(1 << log_n) - 3] = P          # in the last block
+            gc.set_input(bad); gc.evaluate()
+            torch.cuda.synchronize()
+            assert gc.flags() == 1
+            gc.close()
+    monkeypatch.delenv("VC_NO_EVAL_LOCAL", raising=False)
+
+
 def test_run_host_end_to_end_matches(vc):
     import torch
     c = W.config(1)
