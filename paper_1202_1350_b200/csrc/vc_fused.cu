@@ -118,6 +118,7 @@ __device__ __forceinline__ void eval_grid_barrier(unsigned int *cnt, uint32_t &g
 #ifndef VC_EVAL_LOC_LOG
 #define VC_EVAL_LOC_LOG 13
 #endif
+constexpr int EVAL_LOC_MAX = 32;                       // layers of a local run at most
 constexpr uint32_t EVAL_LOC_LOG = VC_EVAL_LOC_LOG;                   // inputs per block of the local run (two tables of 2^13 words: one wave of 128 blocks at n = 2^20)
 __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint32_t d, const uint64_t *in, uint64_t *out0,
                                                           DevState *st, int top, uint32_t loc_bl, int loc_top) {
@@ -130,21 +131,37 @@ __global__ void __launch_bounds__(EVAL_T, 1) k_eval_all(const LayerPlan *L, uint
         uint64_t *Vd = const_cast<uint64_t *>(L[d].V);
         const uint32_t nblk = 1u << (L[d].log_n - loc_bl), B = 1u << loc_bl;
         unsigned bad = 0;
+        // the plans of the local layers sit in global memory: one fetch per kernel, not one dependent L2 round trip per layer
+        __shared__ uint64_t *s_V[EVAL_LOC_MAX];
+        __shared__ uint32_t s_tree[EVAL_LOC_MAX], s_t0[EVAL_LOC_MAX];
+        if (tid < (uint32_t)((int)d - loc_top)) {
+            const LayerPlan &Lp = L[(int)d - 1 - (int)tid];
+            s_V[tid] = const_cast<uint64_t *>(Lp.V); s_tree[tid] = Lp.wiring == W_TREE; s_t0[tid] = Lp.type0;
+        }
+        __syncthreads();
         for (uint32_t blk = b; blk < nblk; blk += G) {
             uint64_t *cur = ev_sm, *nxt = ev_sm + B;
-            for (uint32_t u = tid; u < B; u += EVAL_T) {
-                const uint64_t w = in[(size_t)blk * B + u];
-                bad |= (w >= fp61::P);
-                Vd[(size_t)blk * B + u] = w;
-                cur[u] = w;
+            {   // all of the block's input loads in flight before the first use (B / EVAL_T <= 8 words per thread, 16 B each)
+                constexpr uint32_t NV = (1u << EVAL_LOC_LOG) / (2 * EVAL_T);
+                const ulonglong2 *in2 = reinterpret_cast<const ulonglong2 *>(in + (size_t)blk * B);
+                ulonglong2 *Vd2 = reinterpret_cast<ulonglong2 *>(Vd + (size_t)blk * B), *cur2 = reinterpret_cast<ulonglong2 *>(cur);
+                ulonglong2 w[NV];
+#pragma unroll
+                for (uint32_t k = 0; k < NV; k++) w[k] = in2[k * EVAL_T + tid];
+#pragma unroll
+                for (uint32_t k = 0; k < NV; k++) {
+                    bad |= (w[k].x >= fp61::P) | (w[k].y >= fp61::P);
+                    Vd2[k * EVAL_T + tid] = w[k];
+                    cur2[k * EVAL_T + tid] = w[k];
+                }
             }
             __syncthreads();
             uint32_t share = B;                          // this block's entries of the layer below
             for (int l = (int)d - 1; l >= loc_top; l--) {
-                const bool tree = L[l].wiring == W_TREE;
-                const uint32_t t0 = L[l].type0;
+                const bool tree = s_tree[(int)d - 1 - l] != 0;
+                const uint32_t t0 = s_t0[(int)d - 1 - l];
                 if (tree) share >>= 1;
-                uint64_t *Vo = const_cast<uint64_t *>(L[l].V) + (size_t)blk * share;
+                uint64_t *Vo = s_V[(int)d - 1 - l] + (size_t)blk * share;
                 for (uint32_t g = tid; g < share; g += EVAL_T) {
                     const uint64_t v = tree ? gate_f(t0, cur[2 * g], cur[2 * g + 1]) : gate_f(t0, cur[g], cur[g]);
                     nxt[g] = v; Vo[g] = v;
@@ -523,7 +540,7 @@ static int fused_init_impl(vc_circuit *c, FusedHost &fh) {
         if (ok && c->log_input > EVAL_LOC_LOG && !getenv("VC_NO_EVAL_LOCAL")) {
             uint32_t share_log = EVAL_LOC_LOG;
             int l = (int)c->d - 1;
-            for (; l >= (int)c->first_pair_layer(); l--) {
+            for (; l >= (int)c->first_pair_layer() && (int)c->d - 1 - l < EVAL_LOC_MAX; l--) {
                 const uint32_t w = c->wiring[l];
                 if (w == 1 && c->logs[l] + 1 == c->logs[l + 1] && share_log > 0) share_log--;
                 else if (!(w == 2 && c->logs[l] == c->logs[l + 1])) break;
