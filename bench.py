@@ -62,6 +62,19 @@ def algorithmic_counts(c):
                 modmul=sum(l["modmul"] + l["modmul_eval"] for l in per_layer))
 
 
+def csrc_digest() -> str:
+    """SHA-256 over the kernel sources (csrc/*, include/vc.h, sorted by name): ties profiles/r02_traffic.json to a build."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_1202_1350_b200", "csrc")
+    for name in sorted(os.listdir(base)):
+        with open(os.path.join(base, name), "rb") as f:
+            h.update(name.encode()); h.update(f.read())
+    with open(os.path.join(ROOT, "include", "vc.h"), "rb") as f:
+        h.update(b"vc.h"); h.update(f.read())
+    return h.hexdigest()
+
+
 def measured_peaks():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -358,8 +371,11 @@ def run_ours(args):
             with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
                 tj = json.load(f)
             if k == 2 and args.schedule == 0 and tj.get("kernel_kind") == dom:
-                traffic = int(tj["dram_bytes_read"]) + int(tj["dram_bytes_write"])
-                traffic_src = f"profiles/r02_traffic.json (ncu --set full capture of commit {tj.get('commit', '?')}, one launch)"
+                if tj.get("csrc_sha256") == csrc_digest():    # the capture is of THIS kernel source: else no traffic figure
+                    traffic = int(tj["dram_bytes_read"]) + int(tj["dram_bytes_write"])
+                    traffic_src = f"profiles/r02_traffic.json (ncu --set full capture of commit {tj.get('commit', '?')}, same csrc/ + vc.h digest as this build, one launch)"
+                else:
+                    traffic_src = "profiles/r02_traffic.json is of another kernel source (csrc digest differs): no traffic figure for this build"
         except Exception:
             pass
         roofline = {"bound": "hbm" if dom_hbm_ms >= dom_alu_ms else "alu", "kernel": dom,
