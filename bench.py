@@ -254,6 +254,52 @@ def run_ours(args):
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
+    if args.round_trace:                         # -DVC_TRACE builds only: where the cycles of the wide (k_fused<4>) rounds go, as CTA 0 sees them
+        from collections import defaultdict
+        for _ in range(3):
+            step()
+            torch.cuda.synchronize()
+        n = 60000
+        h = np.zeros(n, dtype=np.uint64)
+        assert L.vc_debug_trace(gc.handle, h.ctypes.data, n, None) == 0
+        codes = (h >> np.uint64(48)).astype(np.int64)
+        clk = (h & np.uint64((1 << 48) - 1)).astype(np.int64)
+        if not codes.any():
+            print("no trace words: build with VC_NVCC_EXTRA=-DVC_TRACE (paper_1202_1350_b200/build.py)")
+            gc.close()
+            return
+        end = int(np.argmax(codes == 0)) if (codes == 0).any() else n
+        names = {("L", 11): "set-up (beta, gate state, start claim)", (11, 12): "barrier", (12, 13): "level build / phase switch", (13, 14): "barrier: level j ready",
+                 (14, 21): "gate loop (a4 + pending a6)", (21, 15): "commit", (15, 16): "barrier + rendezvous + barrier", (16, 13): "fold of level j (+ publish)",
+                 (16, 12): "phase switch (eq tables, phase-2 state)", (16, 17): "after the last round", (17, 70): "line restriction: start",
+                 (70, 71): "line: points l(t)", (71, 72): "line: 8 words -> cubic -> P points per thread", (72, 73): "line: barrier", (73, 74): "line: block fold tree",
+                 (74, 75): "line: Lagrange continuation", (75, 76): "line: eq weight + accumulate", (76, 72): "line: next block", (76, 18): "line: grid all-reduce",
+                 (18, 19): "line_finish (tau, z, claim)"}
+        layer, prev, acc, out = -1, None, None, []
+        for cd, t in zip(codes[:end], clk[:end]):
+            if cd >= 100 + c.d:                  # not a mark: the end of what this launch wrote
+                break
+            if cd >= 100:                        # 100 + layer: a layer starts
+                if layer >= 0:
+                    out.append((layer, acc))
+                layer, acc, prev = int(cd) - 100, defaultdict(lambda: [0, 0]), (int(cd), int(t))
+                continue
+            if prev is None:
+                continue
+            key = ("L" if prev[0] >= 100 else prev[0], int(cd))
+            acc[key][0] += 1
+            acc[key][1] += int(t) - prev[1]
+            prev = (int(cd), int(t))
+        if layer >= 0:
+            out.append((layer, acc))
+        print("SM-clock cycles between trace marks of CTA 0, last launch of the proof (the wide layers); codes: vc_fused_wide.cuh VC_TR(n), 70..76 = line restriction")
+        for layer, d in out:
+            tot = sum(v[1] for v in d.values())
+            print(f"layer {layer}: {tot} cycles")
+            for (a_, b_), (cnt, cyc) in sorted(d.items(), key=lambda kv: -kv[1][1]):
+                print(f"   {str(a_):>3}->{b_:<3} n={cnt:3d} avg={cyc / cnt:8.0f} sum={cyc:8d} {100 * cyc / tot:5.1f}%  {names.get((a_, b_), '')}")
+        gc.close()
+        return
     if args.layer_times:                         # per-layer device time of warm proofs (%globaltimer stamps of the fused kernels): not a bench value
         best = None
         for _ in range(5):
@@ -458,6 +504,7 @@ def main():
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--hosted-chunk-log", type=int, default=0, help="time the copy-every-message approach (SURVEY.md §8f NEXT-3): records and weights in pinned host memory, streamed per message in pieces of 2^N gates")
+    ap.add_argument("--round-trace", action="store_true", help="with a -DVC_TRACE build: cycles between the trace marks of the wide layers' rounds (CTA 0), and exit")
     ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")
     ap.add_argument("--paper-scale", default="", help="f2:N | f0:N | matmul:LOG_M | matmuleq:LOG_M (the single-output circuit of PAPER.md:230) | f2sum:N | f0sum:N (the paper's circuits with ONE sum gate of fan-in n at the output, PAPER.md:220) | pm:LOG_T — time a construction at another size (e.g. f2:23, f0:21, matmul:8, pm:19) instead of a BASELINE.json config; no CPU baseline")
     ap.add_argument("--f2-log-n", type=int, default=0, help="time the F2 construction at n = 2^N instead of a BASELINE.json config (implies --no-cpu-baseline)")
