@@ -476,8 +476,28 @@ def test_run_host_end_to_end_matches(vc):
     h_in = torch.from_numpy(c.input.view(np.int64)).pin_memory()
     h_out = torch.zeros(gc.n_out, dtype=torch.int64).pin_memory()
     h_tr = torch.zeros(gc.words, dtype=torch.int64).pin_memory()
-    for _ in range(2):           # twice: the handle is reusable
+    for _ in range(4):           # the handle is reusable
+        h_out.zero_(); h_tr.zero_()
         vc.vc_run_host(gc.handle, h_in, seed, h_out, h_tr)
         assert np.array_equal(h_out.numpy().view(np.uint64), want_out)
         assert np.array_equal(h_tr.numpy().view(np.uint64), want_tr)
+    # same buffers, other contents
+    x2 = c.input.copy(); x2[::7] = (x2[::7] + np.uint64(5)) % np.uint64(P)
+    want_out2, want_tr2, _, _ = oracle.OracleCircuit(c).prove(x2, seed)
+    h_in.copy_(torch.from_numpy(x2.view(np.int64)))
+    vc.vc_run_host(gc.handle, h_in, seed, h_out, h_tr)
+    assert np.array_equal(h_out.numpy().view(np.uint64), want_out2) and np.array_equal(h_tr.numpy().view(np.uint64), want_tr2)
+    assert not np.array_equal(want_tr2, want_tr)
+    # another seed; then a non-canonical word is reported by this call and not by the next one
+    want_out3, want_tr3, _, _ = oracle.OracleCircuit(c).prove(x2, seed + 1)
+    for _ in range(3):
+        vc.vc_run_host(gc.handle, h_in, seed + 1, h_out, h_tr)
+        assert np.array_equal(h_tr.numpy().view(np.uint64), want_tr3)
+    h_in[3] = -1                 # 2^64 - 1 >= p
+    with pytest.raises(vc.VCError) as e:
+        vc.vc_run_host(gc.handle, h_in, seed + 1, h_out, h_tr)
+    assert e.value.code == 1
+    h_in.copy_(torch.from_numpy(x2.view(np.int64)))
+    vc.vc_run_host(gc.handle, h_in, seed + 1, h_out, h_tr)
+    assert np.array_equal(h_tr.numpy().view(np.uint64), want_tr3)
     gc.close()
