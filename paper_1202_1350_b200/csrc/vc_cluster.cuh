@@ -1,4 +1,4 @@
-// vc_cluster.cuh — layers of at most 2^13 gates proved by ONE thread-block cluster (steps a2-a7).
+// vc_cluster.cuh — layers of at most 2^12 gates (CL_MAX_N) proved by ONE thread-block cluster (steps a2-a7).
 //
 // Same method as every other schedule (each gate contributes independently to each message, the
 // contributions are reduced in F_p).  What this engine changes is the cost of the 2s strictly dependent
@@ -17,7 +17,7 @@
 //     V_{i+1}: the CTA folds its own block for levels < m, the A blocks' last pairs are gathered into every CTA with
 //     the commit of round m-1 (st.async), and from level m on every CTA folds the whole (<= 32-entry) table itself.
 //     Irregular wiring: every CTA holds the whole table (m = s);
-//   * the line restriction (a7) is STREAMED through phase 2 by four line warps: the fold tree of V_{i+1} along
+//   * the line restriction (a7) is STREAMED through phase 2 by two line warps (16, 17): the fold tree of V_{i+1} along
 //     l(t) = r1 + t (r2 - r1) needs challenge r2_k for its level k only, so level k is folded as soon as round k of
 //     phase 2 has been handed off (a per-thread cubic over variables 0..2, continued to t = 2..s by finite differences,
 //     then one multiply per (node, t) and level).  When the last challenge arrives one fold is left and q[2..s] follow
@@ -308,7 +308,6 @@ __device__ __forceinline__ void cl_rounds(const ClArgs &a, ClShared &S, uint8_t 
     const bool gate_thr = tid < CL_GW, has_ign = Lp.has_relay != 0;
     const uint32_t ft = tid - CL_GW;                         // fold thread number (fold threads only)
     const uint32_t pidx = gate_thr ? tid : ngt + ft;         // number among the np participants
-    const uint64_t *__restrict__ Vb = S.pl[layer - a.begin].Vb;
     FusedCtx &cx = S.cx;
     const uint64_t seed = cx.seed;
     const uint32_t ctr0 = (uint32_t)cx.ctr;

@@ -360,24 +360,9 @@ __device__ __forceinline__ void reducer_housekeeping(const FusedArgs &a, uint32_
     }
 }
 __device__ __forceinline__ void reducer_post(const FusedArgs &a, uint32_t ep, uint64_t t0, uint64_t t1, uint64_t t2, uint64_t *tr,
-                                             RoundPend &pd) {
-    const uint32_t lane = threadIdx.x & 31;
-    unsigned long long *slot = a.slots + (size_t)(ep % F_RING) * F_SLOT_WORDS;
-    if (lane >= 1 && lane < 7) {
-        const uint32_t k = (lane - 1) >> 1;
-        const uint64_t v = k == 0 ? t0 : (k == 1 ? t1 : t2);
-        red_add(slot + lane, (((lane - 1) & 1) ? (v >> 32) : (v & 0xffffffffull)) | F_CNT_ONE);
-    }
-    if (blockIdx.x == 0) {
-        if (pd.tr2) round_slot_to_transcript(a.slots + (size_t)pd.s2 * F_SLOT_WORDS, pd.tr2, lane);
-        pd.tr2 = pd.tr1; pd.s2 = pd.s1; pd.tr1 = tr; pd.s1 = ep % F_RING;
-    }
-    if (blockIdx.x == gridDim.x - 1) {   // slot recycling is the last CTA's job (CTA 0 already has the transcript)
-        unsigned long long *z = a.slots + (size_t)((ep + 2) % F_RING) * F_SLOT_WORDS;
-#pragma unroll
-        for (int q = 0; q < F_SLOT_WORDS / 32; q++) z[q * 32 + lane] = 0ull;
-        __threadfence();
-    }
+                                             RoundPend &pd) {     // the thin path's reducer warp does both jobs
+    reducer_post_data(a, ep, t0, t1, t2);
+    reducer_housekeeping(a, ep, tr, pd);
 }
 __device__ __forceinline__ void reducer_flush(const FusedArgs &a, RoundPend &pd) {
     const uint32_t lane = threadIdx.x & 31;

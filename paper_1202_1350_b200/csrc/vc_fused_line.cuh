@@ -55,7 +55,6 @@ __device__ __noinline__ void line_partials(const uint64_t *Vb, uint32_t s, Fused
     uint64_t *A = pts + ((((size_t)s + 1) * sp + 1) & ~(size_t)1);
     uint64_t *B = A + (size_t)NB * P;
     uint64_t *fx = B + (((size_t)NB * P + 1) / 2 + 1 & ~(size_t)1);
-    uint64_t *dl = fx + 32;
     VC_TRL(70);
     for (uint32_t i = tid; i < m; i += nthr) cx.acc[i] = 0;
     {   // lane k of every warp owns variable k (sp <= 30); warp w takes t = w, w + nw, ...: l(t + nw) = l(t) + nw d, no division

@@ -1,4 +1,4 @@
-// vc_fused_small.cuh — one narrow layer (<= 2^10 gates, table <= 2^12 words) proved by a single CTA out of shared
+// vc_fused_small.cuh — one narrow layer (<= 2^8 gates: F_SMALL_N_LOG, table <= 2^12 words) proved by a single CTA out of shared
 // memory (steps a2-a7).  One gate per thread in registers; only as many warps as the layer needs take part and they
 // synchronise on a named barrier, so a round of a 1-gate layer costs two 1-warp barriers, not two 32-warp ones.
 // Per round: contributions -> 3 warp REDUX sums -> barrier (message complete) -> challenge -> weight update and

@@ -290,7 +290,6 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
     __syncthreads();
     uint32_t ep = cx.epoch;
     RoundPend pd; pd.tr1 = pd.tr2 = nullptr; pd.s1 = pd.s2 = 0;
-    bool first = true;
     for (int ph = 0; ph < 2; ph++) {
         const uint32_t mode = Lp.mode[ph], K = Lp.K[ph], blo = cp.blo[ph], nbk = cp.nb[ph];
         uint64_t *rr = ph == 0 ? cx.r1 : cx.r2;
@@ -457,7 +456,7 @@ __device__ __forceinline__ void wide_layer(const FusedArgs &a, FusedCtx &cx, con
             }
             __syncthreads();
             VC_TR(16);
-            ctr++; tr += 3; ep++; first = false;
+            ctr++; tr += 3; ep++;
             r_prev = *rslot;
         }
         // ---- V~_{i+1}(r) = the two entries of level s-1 folded with the last challenge
