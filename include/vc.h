@@ -23,7 +23,8 @@ extern "C" {
 
 typedef struct vc_circuit vc_circuit; /* opaque; owns device copies of records, V tables, scratch, proof state */
 
-enum { VC_OK = 0, VC_ERR_ARG = 1, VC_ERR_SHAPE = 2, VC_ERR_STATE = 3, VC_ERR_CUDA = 4, VC_ERR_NOMEM = 5 };
+enum { VC_OK = 0, VC_ERR_ARG = 1, VC_ERR_SHAPE = 2, VC_ERR_STATE = 3, VC_ERR_CUDA = 4, VC_ERR_NOMEM = 5,
+       VC_ERR_LIMIT = 6 /* a size beyond the fixed maximum of an entry point that allocates nothing */ };
 enum { VC_ADD = 0, VC_MULT = 1, VC_SUB = 2, VC_RELAY = 3, VC_SUM = 4 };
 
 /* VC_SUM — the "single sum-gate of very large fan-in at the output" (DESIGN.md
@@ -154,6 +155,28 @@ int vc_status(const vc_circuit *c, uint32_t *h_flags, void *cuda_stream);
  * VC_K_FUSED_THIN, VC_K_FUSED_WIDE (bench.py uses it to give every kernel kind its own algorithmic byte count);
  * VC_ERR_STATE when the circuit has no fused plan (streaming schedule only) */
 int vc_debug_layer_kinds(const vc_circuit *c, uint32_t *h_kind);
+/* vc_mle_device_noalloc — the multilinear extension of a device table at one point, for callers that cannot allocate
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The operation is the verifier's
+ * "secret" of PAPER.md:127 (§4.1.2) / :99: out = sum_u eq(u, x) V[u] over the 2^log_n words of V, every element one
+ * chi-weighted term, reduced in F_p — the same arithmetic as the start-claim and closing-check kernels of
+ * vc_verify_transcript_device, whose scratch is cudaMalloc'd per circuit.  Here the kernel's scratch (block partials,
+ * ticket, status word) is one file-scope device array of VC_NOALLOC_SCRATCH_WORDS 64-bit words (4 KB) that every GPU
+ * loading the library holds until the process exits; the call itself calls no cudaMalloc / cudaFree / allocating routine:
+ * it enqueues one 16-byte memset of the scratch's ticket and status words, one kernel and one 8-byte device-to-device
+ * copy on cuda_stream and returns without synchronising.
+ *   d_values  DEVICE, 2^log_n words (read); a word >= p is reduced by masking to 61 bits and reported in d_out2[1]
+ *   log_n     0 .. VC_NOALLOC_MAX_LOG (28: tables of up to 2^28 words = 2 GiB); larger: VC_ERR_LIMIT, nothing enqueued
+ *   d_point   DEVICE, log_n canonical words x[0..log_n) (read; bit k of the index is variable k); may be NULL if log_n = 0
+ *   d_out2    DEVICE, 2 words (written): [0] = the value, [1] = 1 if a word of d_values was >= p, else 0
+ * The first call on a device resolves the scratch array's device address (cudaGetSymbolAddress, once per device, with that
+ * device current): make one call outside any stream capture first.  All calls on a device SHARE the array: calls that
+ * overlap on the GPU (different streams, several host threads) race — serialise them on one stream or with events.
+ * Errors: VC_ERR_ARG (null pointer), VC_ERR_LIMIT (log_n too large), VC_ERR_CUDA. */
+#define VC_NOALLOC_MAX_LOG 28
+#define VC_NOALLOC_SCRATCH_WORDS 512
+int vc_mle_device_noalloc(const uint64_t *d_values, uint32_t log_n, const uint64_t *d_point, uint64_t *d_out2,
+                          void *cuda_stream);
+
 /* how the prover obtains each layer's wiring (the paper's §5.1.4 computes the tree's indices instead of
  * loading them): h_mode receives d words, 0 = the stored records are read, 1 = binary tree (2g, 2g+1) computed, 2 = in1 = in2 = g
  * computed, 3 = computed from the bit-field rule vc_load fitted to the records and checked against every one of them.  The

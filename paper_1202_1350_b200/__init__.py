@@ -8,7 +8,7 @@ There is no CPU fallback: importing works anywhere, calling needs the built libr
 from .binding import (  # noqa: F401
     VCError, Circuit, lib, library_path,
     vc_circuit_load, vc_evaluate, vc_prove_layer, vc_prove, vc_run_host, vc_verify_transcript,
-    vc_verify_transcript_device, vc_debug_verifier_sums,
+    vc_verify_transcript_device, vc_debug_verifier_sums, vc_mle_device_noalloc,
     vc_circuit_free, vc_strerror, vc_transcript_words, vc_total_transcript_words,
-    VC_OK, VC_ERR_ARG, VC_ERR_SHAPE, VC_ERR_STATE, VC_ERR_CUDA, VC_ERR_NOMEM,
+    VC_OK, VC_ERR_ARG, VC_ERR_SHAPE, VC_ERR_STATE, VC_ERR_CUDA, VC_ERR_NOMEM, VC_ERR_LIMIT,
 )

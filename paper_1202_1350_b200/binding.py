@@ -6,7 +6,7 @@ from pathlib import Path
 
 import numpy as np
 
-VC_OK, VC_ERR_ARG, VC_ERR_SHAPE, VC_ERR_STATE, VC_ERR_CUDA, VC_ERR_NOMEM = range(6)
+VC_OK, VC_ERR_ARG, VC_ERR_SHAPE, VC_ERR_STATE, VC_ERR_CUDA, VC_ERR_NOMEM, VC_ERR_LIMIT = range(7)
 
 _HERE = Path(__file__).resolve().parent
 _SO = _HERE / "libvc.so"
@@ -16,7 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
-    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring", "vc_circuit_load_hosted", "vc_debug_hosted_bytes",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring", "vc_circuit_load_hosted", "vc_debug_hosted_bytes", "vc_mle_device_noalloc",
 ]
 
 
@@ -74,6 +74,7 @@ def lib():
             "vc_debug_layer_wiring": (i32, [vp, vp]),
             "vc_circuit_load_hosted": (i32, [vp, u32, u32, u32, vp]),
             "vc_debug_hosted_bytes": (i32, [vp, vp, vp]),
+            "vc_mle_device_noalloc": (i32, [vp, u32, vp, vp, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
         }
@@ -134,6 +135,12 @@ def vc_circuit_load(layers, log_input: int, hosted_chunk_log=None) -> int:
     else:
         _check(lib().vc_circuit_load_hosted(arr, len(layers), int(log_input), int(hosted_chunk_log), C.byref(h)), "vc_circuit_load_hosted")
     return h.value
+
+
+def vc_mle_device_noalloc(d_values, log_n: int, d_point, d_out2, stream=None):
+    """Enqueue out2 = (V~(point), status) for the 2^log_n-word device table d_values; allocates nothing (include/vc.h)."""
+    _check(lib().vc_mle_device_noalloc(_dev_ptr(d_values), int(log_n), _dev_ptr(d_point), _dev_ptr(d_out2), _stream_ptr(stream)),
+           "vc_mle_device_noalloc")
 
 
 def vc_evaluate(handle: int, d_input, d_outputs=None, stream=None):

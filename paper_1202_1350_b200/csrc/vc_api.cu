@@ -52,6 +52,7 @@ extern "C" const char *vc_strerror(int code) {
     case VC_ERR_STATE: return "call out of order (vc_evaluate, then vc_prove_layer 0..d-1 with one seed)";
     case VC_ERR_CUDA: return "CUDA error (no device, launch or copy failure)";
     case VC_ERR_NOMEM: return "out of memory";
+    case VC_ERR_LIMIT: return "size beyond the fixed maximum of an entry point that allocates nothing (vc_mle_device_noalloc: log_n <= 28)";
     default: return "unknown error";
     }
 }

@@ -345,3 +345,90 @@ extern "C" int vc_debug_verifier_sums(const vc_circuit *c, uint64_t *h_sums, uin
         if (p.first == c) { std::memcpy(h_sums, p.second->h_pin + c->total_words, n * 8); return VC_OK; }
     return VC_ERR_STATE;
 }
+
+namespace vc {
+// ------------------------------------------------------------------------------------------------------------------
+// vc_mle_device_noalloc — the multilinear extension of a device table at one point (the verifier's "secret", PAPER.md:127
+// §4.1.2: one chi-weighted term per element, reduced in F_p) for callers that cannot allocate: code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arithmetic as k_v_mle above; what differs is
+// where the kernel's scratch lives: the block partials, the last-block ticket and the status word sit in ONE file-scope
+// device array of fixed size instead of the per-circuit cudaMalloc'd scratch of verifier_of().  Every GPU that loads the
+// library holds these VC_NOALLOC_SCRATCH_WORDS * 8 = 4 KB until the process exits.
+//
+// In host code `g_noalloc_scratch` is a host-side stand-in, not a device address, so the host never passes the name to a
+// kernel: once per device, with that device current, noalloc_scratch() asks cudaGetSymbolAddress for the address and keeps it.
+// Every call on a device shares the array and finds the previous call's contents in it: the ticket and status words are
+// cleared on the caller's stream before each launch (the partials are rewritten before they are read).  Calls that
+// overlap on the GPU (two streams, two host threads) race on the array: serialise them.
+constexpr uint32_t NA_PART = 0;                           // [0, V_MAX_BLOCKS): one partial per block
+constexpr uint32_t NA_TICKET = V_MAX_BLOCKS;              // low 32 bits: last-block ticket
+constexpr uint32_t NA_BAD = V_MAX_BLOCKS + 1;             // low 32 bits: 1 = a word >= p was seen
+static_assert(NA_BAD < VC_NOALLOC_SCRATCH_WORDS, "scratch array too small for the partials");
+static __device__ __align__(256) unsigned long long g_noalloc_scratch[VC_NOALLOC_SCRATCH_WORDS];
+
+// k_v_mle with its scratch taken from one array: out[0] = sum_u eq(u, x) V[u] over 2^s words
+__global__ void __launch_bounds__(VT) k_v_mle_static(const uint64_t *__restrict__ V, uint32_t s, const uint64_t *__restrict__ x,
+                                                       unsigned long long *scratch, uint64_t *out) {
+    extern __shared__ __align__(16) uint64_t vsm[];
+    __shared__ uint64_t red[32], xs[MAX_VARS];
+    uint64_t *part = reinterpret_cast<uint64_t *>(scratch + NA_PART);
+    unsigned *ticket = reinterpret_cast<unsigned *>(scratch + NA_TICKET), *bad = reinterpret_cast<unsigned *>(scratch + NA_BAD);
+    const uint32_t tid = threadIdx.x;
+    if (tid < s) xs[tid] = x[tid];
+    __syncthreads();
+    const EqTab e = build_eq_tab(vsm, vsm + (2u << V_EQLOG), xs, s, tid);
+    __syncthreads();
+    const uint64_t n = 1ull << s;
+    acc128 A; A.clear();
+    uint64_t sum = 0; uint32_t cnt = 0; unsigned nc = 0;
+    for (uint64_t u = (uint64_t)blockIdx.x * VT + tid; u < n; u += (uint64_t)gridDim.x * VT) {
+        const uint64_t w = __ldg(V + u);
+        nc |= w >= fp61::P;
+        A.mac(e.eq_of((uint32_t)u), w & fp61::P);
+        if (++cnt == 32) { sum = fp61::add(sum, A.value()); A.clear(); cnt = 0; }
+    }
+    if (nc) atomicOr(bad, 1u);
+    uint64_t v[1] = {fp61::add(sum, A.value())};
+    verifier_reduce<1>(v, red, part, ticket, out);
+}
+
+constexpr int NA_MAX_DEVICES = 64;
+static unsigned long long *g_noalloc_ptr[NA_MAX_DEVICES];  // per device: the array's DEVICE address (null: not asked yet)
+static std::mutex g_noalloc_mutex;
+
+// set-up, once per device, with that device current: the device address of the scratch array
+static int noalloc_scratch(unsigned long long **p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NA_MAX_DEVICES) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    std::lock_guard<std::mutex> lk(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        unsigned long long *q = nullptr;
+        if (cudaGetSymbolAddress((void **)&q, g_noalloc_scratch) != cudaSuccess || !q) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+        g_noalloc_ptr[dev] = q;
+    }
+    *p = g_noalloc_ptr[dev];
+    return VC_OK;
+}
+
+}  // namespace vc
+
+extern "C" int vc_mle_device_noalloc(const uint64_t *d_values, uint32_t log_n, const uint64_t *d_point, uint64_t *d_out2,
+                                     void *cuda_stream) {
+    using namespace vc;
+    if (!d_values || !d_out2 || (log_n > 0 && !d_point)) return VC_ERR_ARG;
+    if (log_n > VC_NOALLOC_MAX_LOG) return VC_ERR_LIMIT;       // beyond the stated maximum: nothing is enqueued
+    unsigned long long *scr = nullptr;
+    const int rc = noalloc_scratch(&scr);
+    if (rc != VC_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the array keeps the last call's contents: ticket and status start at zero (adjacent words: one memset node)
+    if (cudaMemsetAsync(scr + NA_TICKET, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    const uint64_t n = 1ull << log_n;
+    const unsigned blocks = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((n + VT - 1) / VT, (uint64_t)V_MAX_BLOCKS));
+    k_v_mle_static<<<blocks, VT, V_TAB_WORDS * 8, st>>>(d_values, log_n, d_point, scr, d_out2);   // (not VC_LAUNCH: its profiling mode creates events)
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (cudaGetLastError() != cudaSuccess) return VC_ERR_CUDA;
+    // d_out2[1] <- the status word (0 / 1), device to device on the same stream
+    if (cudaMemcpyAsync(d_out2 + 1, scr + NA_BAD, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; }
+    return VC_OK;
+}
