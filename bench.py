@@ -237,6 +237,7 @@ def run_ours(args):
     L = vc.lib()
     gc = vc.Circuit(c, hosted_chunk_log=args.hosted_chunk_log or None)
     if args.hosted_chunk_log:
+        gc.set_hosted_weights(args.hosted_swap)
         args.schedule = 2                        # the one schedule of a hosted handle (copy-every-message)
     gc.set_schedule(args.schedule)
     gc.set_input(c.input)
@@ -494,8 +495,8 @@ def run_ours(args):
                 "roofline": roofline, "cpu_baseline": cpu, "verifier": verifier}
         if args.hosted_chunk_log:                # copy-every-message: the per-message traffic over the host link, inside the timed steps
             hb = gc.hosted_bytes()
-            line["hosted"] = {"chunk_log": args.hosted_chunk_log, "proof_h2d_bytes": hb[0], "proof_d2h_bytes": hb[1],
-                              "note": "records and weights streamed from pinned host memory for every message (PAPER.md:165); counted on top of e2e's input/output copies"}
+            line["hosted"] = {"chunk_log": args.hosted_chunk_log, "weights": "swapped through host memory" if args.hosted_swap else "recomputed per message", "proof_h2d_bytes": hb[0], "proof_d2h_bytes": hb[1],
+                              "note": "records (and, with --hosted-swap, weights) streamed from pinned host memory for every message (PAPER.md:165); counted on top of e2e's input/output copies"}
         print(json.dumps(line), flush=True)
     gc.close()
     if world > 1:
@@ -511,6 +512,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--schedule", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--hosted-swap", action="store_true", help="with --hosted-chunk-log: swap the weights through host memory per message (the paper's wording) instead of recomputing them on the device")
     ap.add_argument("--hosted-chunk-log", type=int, default=0, help="time the copy-every-message approach (SURVEY.md §8f NEXT-3): records and weights in pinned host memory, streamed per message in pieces of 2^N gates")
     ap.add_argument("--round-trace", action="store_true", help="with a -DVC_TRACE build: cycles between the trace marks of the wide layers' rounds (CTA 0), and exit")
     ap.add_argument("--layer-times", action="store_true", help="print the per-layer device times of a warm proof (fused schedule) and exit")

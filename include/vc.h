@@ -58,13 +58,18 @@ int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_c
  * the per-gate data — records (9 B per gate) and weights (8 B per gate) — stays in pinned HOST memory (the record arrays
  * are copied once into the handle and page-locked there); the device holds the value tables, the fold tables and two chunk
  * slots of 2^chunk_log gates (8 <= chunk_log <= 28, else VC_ERR_ARG).  For EVERY message of a layer the whole layer
- * is streamed through the slots piece by piece: H2D of a piece's records and weights, the piece's contribution to the
- * message (with the pending weight update of the previous challenge applied first), D2H of its updated weights, the
- * copies of neighbouring pieces overlapping the kernel on two internal streams.  vc_evaluate streams the records once per
+ * is streamed through the slots piece by piece: H2D of a piece's records, the piece's contribution to the message, the
+ * copies of neighbouring pieces overlapping the kernel on internal streams.  The weights are either recomputed from the
+ * record for every message (default: nothing but 9 B per gate and message crosses the host link) or swapped through the
+ * host array as the paper words it (vc_hosted_set_weights(c, 1): + 8 B per gate up and 8 B down per message, the pending
+ * update of the previous challenge applied when the piece comes back).  vc_evaluate streams the records once per
  * layer.  Every other call (vc_prove_layer, vc_prove, vc_run_host, vc_verify_transcript, sizes) behaves as for a resident
  * circuit and produces the same words; vc_set_schedule accepts only 2 for such a handle (and 2 only for such a handle),
  * vc_verify_transcript_device returns VC_ERR_STATE (its wiring sums need device-resident records). */
 int vc_circuit_load_hosted(const vc_layer *layers, uint32_t d, uint32_t log_input, uint32_t chunk_log, vc_circuit **out);
+/* hosted handles only (else VC_ERR_STATE): swap = 0 recompute the weights per message (default), 1 swap them through host
+ * memory.  Takes effect at the next vc_prove_layer; set it before layer 0.  Same transcript either way. */
+int vc_hosted_set_weights(vc_circuit *c, int swap);
 /* bytes a hosted circuit moved over the host link in its last vc_evaluate (h2d only) or since layer 0 of its last proof;
  * VC_ERR_STATE for a resident circuit */
 int vc_debug_hosted_bytes(const vc_circuit *c, uint64_t *h2d, uint64_t *d2h);

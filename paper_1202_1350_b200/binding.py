@@ -16,7 +16,7 @@ EXPORTS = [
     "vc_circuit_free", "vc_strerror", "vc_transcript_words", "vc_total_transcript_words", "vc_depth",
     "vc_log_size", "vc_debug_state", "vc_debug_values", "vc_status", "vc_launch_count", "vc_set_schedule",
     "vc_debug_fieldop", "vc_bench_modmul", "vc_profile_enable", "vc_profile_read", "vc_debug_layer_stamps", "vc_debug_trace",
-    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring", "vc_circuit_load_hosted", "vc_debug_hosted_bytes", "vc_mle_device_noalloc",
+    "vc_verify_transcript_device", "vc_debug_verifier_sums", "vc_debug_layer_kinds", "vc_debug_layer_wiring", "vc_circuit_load_hosted", "vc_debug_hosted_bytes", "vc_hosted_set_weights", "vc_mle_device_noalloc",
 ]
 
 
@@ -74,6 +74,7 @@ def lib():
             "vc_debug_layer_wiring": (i32, [vp, vp]),
             "vc_circuit_load_hosted": (i32, [vp, u32, u32, u32, vp]),
             "vc_debug_hosted_bytes": (i32, [vp, vp, vp]),
+            "vc_hosted_set_weights": (i32, [vp, i32]),
             "vc_mle_device_noalloc": (i32, [vp, u32, vp, vp, vp]),
             "vc_profile_enable": (i32, [i32]),
             "vc_profile_read": (i32, [vp, vp]),
@@ -269,6 +270,10 @@ class Circuit:
         h = np.zeros(self.d, dtype=np.uint32)
         _check(lib().vc_debug_layer_wiring(self.handle, h.ctypes.data), "vc_debug_layer_wiring")
         return h
+
+    def set_hosted_weights(self, swap: bool):
+        """Hosted circuits: recompute the weights per message (False, default) or swap them through host memory (True)."""
+        _check(lib().vc_hosted_set_weights(self.handle, int(bool(swap))), "vc_hosted_set_weights")
 
     def hosted_bytes(self):
         """(h2d, d2h) bytes a hosted circuit moved in its last evaluation / proof (vc_debug_hosted_bytes)."""

@@ -199,6 +199,12 @@ extern "C" int vc_circuit_load_hosted(const vc_layer *layers, uint32_t d, uint32
     if (chunk_log < 8 || chunk_log > 28) return VC_ERR_ARG;
     return load_any(layers, d, log_input, true, chunk_log, out);
 }
+extern "C" int vc_hosted_set_weights(vc_circuit *c, int swap) {
+    if (!c || swap < 0 || swap > 1) return VC_ERR_ARG;
+    if (!c->hosted) return VC_ERR_STATE;
+    c->hosted_swap = swap != 0;
+    return VC_OK;
+}
 extern "C" int vc_debug_hosted_bytes(const vc_circuit *c, uint64_t *h2d, uint64_t *d2h) {
     if (!c || !h2d || !d2h) return VC_ERR_ARG;
     if (!c->hosted) return VC_ERR_STATE;

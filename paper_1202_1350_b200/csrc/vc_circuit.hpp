@@ -43,6 +43,7 @@ struct vc_circuit {
     // through two device slots for every message (the copy-every-message approach)
     bool hosted = false;
     uint32_t chunk_log = 0;
+    bool hosted_swap = false;                   // weights swapped through host memory (the paper's wording) instead of recomputed per message
     std::vector<void *> pinned_ptrs;            // record arrays registered with cudaHostRegister
     uint64_t *p_P = nullptr;                    // pinned host weights, max layer size
     struct HostedSlot { uint8_t *type; uint32_t *in1, *in2; uint64_t *P; cudaEvent_t ready, done, back; };

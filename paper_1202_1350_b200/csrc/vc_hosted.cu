@@ -14,13 +14,18 @@
 //     caller's stream  k_cem_round on chunk k                           |  (events per slot)
 //     copy-out stream  D2H  weights of chunk k-1 back to the host       |
 //
-// The weight update of round j-1 (P[g] *= chi(bit, r_{j-1}), step a6) needs the challenge that only exists once every chunk
-// of round j-1 has been reduced, so it is applied when the chunk comes back for round j, in the same kernel, before the
-// gate's contribution; the updated weights are what travels back.  Round 0 computes the beta weights in place of the H2D
-// of P (a3).  The message of a round is the sum over chunks of the per-chunk sums (a device accumulator; the kernel of the
-// last chunk writes the message and draws the challenge).  Fold tables, line restriction and the sum gate are the
-// resident kernels of the streaming schedule.  Results are bit-identical to the resident schedules
-// (tests/test_gpu_hosted.py compares with the oracle).
+// Two ways to have the weights P[g] = beta(z, g) x (chi factors of the challenges so far) at hand (vc_hosted_set_weights):
+//   recompute (default): the kernel forms P[g] from the record alone - beta by direct product over the bits of g, the chi
+//       factors over the bound bits of in1 (and in2) - up to ~60 multiplies per gate and message, cheap next to 9 B per
+//       gate over the host link, so nothing but the records ever crosses the link: 9 B per gate and message, one direction;
+//   swap (the paper's wording: "swapping each piece back to host memory"): the weights live in a pinned host
+//       array; a piece brings its weights along (8 B per gate up), the kernel applies the pending update of the previous
+//       challenge (it exists only once every piece of the previous message has been reduced) before the gate's
+//       contribution, and the updated weights travel back on the copy-out stream (8 B per gate down): 25 B per gate and message.
+// Round 0 of a layer computes beta either way (a3) and, for layer 0, the start claim.  The message of a round is the sum over
+// pieces of the per-piece sums (a device accumulator; the kernel of the last piece writes the message and draws the
+// challenge).  Fold tables, line restriction and the sum gate are the resident kernels of the streaming schedule.  Results
+// are bit-identical to the resident schedules (tests/test_gpu_hosted.py compares with the oracle, both ways).
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -42,35 +47,44 @@ static inline uint32_t grid_for(uint64_t n, int sm_count, int per_thread = 4) {
 #define H_TRY(x) do { if ((x) != cudaSuccess) { (void)cudaGetLastError(); return VC_ERR_CUDA; } } while (0)
 
 // One chunk of one message.  mode 0: first round of the layer, P[g] = beta(z, g0 + g) computed here (and, for layer 0, the
-// start claim sum beta V_0); mode 1: pending update by the previous round's challenge on bit j-1 of this phase's index;
-// mode 2: first round of phase 2, pending update on bit s-1 of in1.  `last`: this chunk completes the message.
+// start claim sum beta V_0); mode 1: a later round of the same phase; mode 2: first round of phase 2.  `last`: this chunk
+// completes the message.  recompute != 0: P from the record (beta and the chi factors of r1[0..), r2[0..)); else P comes in
+// Pw, gets the pending factor of the previous challenge (bit j-1 of this phase's index; bit s-1 of in1 in mode 2) and goes
+// back through Pw.
 template <int PHASE>
 __global__ void __launch_bounds__(RED_BLOCK)
 k_cem_round(const uint8_t *__restrict__ type, const uint32_t *__restrict__ in1, const uint32_t *__restrict__ in2, uint64_t *__restrict__ Pw,
             uint32_t g0, uint32_t cnt, uint32_t si, const uint64_t *__restrict__ Vi, const uint64_t *__restrict__ tab,
-            const uint64_t *__restrict__ Vb, DevState *st, uint32_t j, uint32_t s, int mode, int last, int set_claim, uint64_t *part,
-            uint64_t *acc, uint64_t *tr) {
+            const uint64_t *__restrict__ Vb, DevState *st, uint32_t j, uint32_t s, int mode, int last, int set_claim, int recompute,
+            uint64_t *part, uint64_t *acc, uint64_t *tr) {
     __shared__ uint64_t red[4 * 32];
-    __shared__ uint64_t zs[MAX_VARS];
-    if (threadIdx.x < MAX_VARS) zs[threadIdx.x] = st->z[threadIdx.x];
+    __shared__ uint64_t zs[MAX_VARS], r1s[MAX_VARS], r2s[MAX_VARS];
+    if (threadIdx.x < MAX_VARS) { zs[threadIdx.x] = st->z[threadIdx.x]; r1s[threadIdx.x] = st->r1[threadIdx.x]; r2s[threadIdx.x] = st->r2[threadIdx.x]; }
     __syncthreads();
     acc128 a0, a1, a2, a3; a0.clear(); a1.clear(); a2.clear(); a3.clear();
     uint64_t s0 = 0, s1 = 0, s2 = 0, s3 = 0; int it = 0;
     const uint64_t v1 = PHASE == 2 ? st->v1 : 0;
     const uint64_t rp = st->r, omrp = fp61::sub(1, rp);
+    const uint32_t n1 = PHASE == 1 ? j : s, n2 = PHASE == 1 ? 0u : j;    // bound bits of in1 / in2 when this message is formed
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < cnt; g += gridDim.x * blockDim.x) {
         const uint32_t t = type[g], i1 = in1[g], i2 = in2[g];
         uint64_t P;
-        if (mode == 0) {
+        if (mode == 0 || recompute) {
             const uint32_t gg = g0 + g;
             P = 1;
             for (uint32_t k = 0; k < si; k++) P = fp61::mul(P, fp61::chi((gg >> k) & 1u, zs[k]));
-            if (set_claim) a3.mac(P, Vi[gg]);
+            if (mode == 0 && set_claim) a3.mac(P, Vi[gg]);
+            if (mode != 0) {
+                uint64_t e1 = 1, e2 = 1;                                 // two more chains, independent of the first
+                for (uint32_t k = 0; k < n1; k++) e1 = fp61::mul(e1, fp61::chi((i1 >> k) & 1u, r1s[k]));
+                for (uint32_t k = 0; k != n2; k++) e2 = fp61::mul(e2, fp61::chi((i2 >> k) & 1u, r2s[k]));
+                P = fp61::mul(P, fp61::mul(e1, e2));
+            }
         } else {
             const uint32_t pb = mode == 1 ? (((PHASE == 1 ? i1 : i2) >> (j - 1)) & 1u) : ((i1 >> (s - 1)) & 1u);
             P = fp61::mul(Pw[g], pb ? rp : omrp);
         }
-        Pw[g] = P;
+        if (!recompute) Pw[g] = P;
         const uint32_t idx = PHASE == 1 ? i1 : i2;
         const uint32_t b = (idx >> j) & 1u, u = idx >> (j + 1);
         const ulonglong2 pr = *reinterpret_cast<const ulonglong2 *>(tab + 2 * (size_t)u);
@@ -229,27 +243,30 @@ int hosted_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d
         const uint64_t *tab = Vb;
         for (uint32_t j = 0; j < s; j++) {
             const int mode = (phase == 1 && j == 0) ? 0 : ((phase == 2 && j == 0) ? 2 : 1);
-            if (mode != 0) H_TRY(cudaStreamWaitEvent(c->s_in, c->ev_round, 0));          // the weights of the previous message are back on the host
+            const bool swap = c->hosted_swap;
+            if (swap && mode != 0) H_TRY(cudaStreamWaitEvent(c->s_in, c->ev_round, 0));  // the weights of the previous message are back on the host
             for (uint32_t q = 0; q < nchunks; q++, k++) {
                 const uint32_t g0 = q * ch, cnt = std::min(ch, n - g0);
                 auto &sl = c->slot[k & 1];
-                if ((rc = chunk_in(c, layer, k, g0, cnt, mode != 0)) != VC_OK) return rc;
+                if ((rc = chunk_in(c, layer, k, g0, cnt, swap && mode != 0)) != VC_OK) return rc;
                 H_TRY(cudaStreamWaitEvent(st, sl.ready, 0));
                 const int last = q + 1 == nchunks, set_claim = layer == 0 && mode == 0;
                 const uint32_t gg = grid_for(cnt, c->sm_count);
                 if (phase == 1)
                     VC_LAUNCH(VC_K_ROUND, k_cem_round<1>, gg, RED_BLOCK, 0, st, sl.type, sl.in1, sl.in2, sl.P, g0, cnt, si, c->d_V[layer], tab, Vb, S, j, s,
-                              mode, last, set_claim, c->d_part, c->d_acc, tr);
+                              mode, last, set_claim, swap ? 0 : 1, c->d_part, c->d_acc, tr);
                 else
                     VC_LAUNCH(VC_K_ROUND, k_cem_round<2>, gg, RED_BLOCK, 0, st, sl.type, sl.in1, sl.in2, sl.P, g0, cnt, si, c->d_V[layer], tab, Vb, S, j, s,
-                              mode, last, set_claim, c->d_part, c->d_acc, tr);
+                              mode, last, set_claim, swap ? 0 : 1, c->d_part, c->d_acc, tr);
                 H_TRY(cudaEventRecord(sl.done, st));
-                H_TRY(cudaStreamWaitEvent(c->s_out, sl.done, 0));                        // swap the piece back
-                H_TRY(cudaMemcpyAsync(c->p_P + g0, sl.P, (size_t)cnt * 8, cudaMemcpyDeviceToHost, c->s_out));
-                c->d2h_bytes += (uint64_t)cnt * 8;
-                H_TRY(cudaEventRecord(sl.back, c->s_out));
+                if (swap) {                                                              // swap the piece back
+                    H_TRY(cudaStreamWaitEvent(c->s_out, sl.done, 0));
+                    H_TRY(cudaMemcpyAsync(c->p_P + g0, sl.P, (size_t)cnt * 8, cudaMemcpyDeviceToHost, c->s_out));
+                    c->d2h_bytes += (uint64_t)cnt * 8;
+                    H_TRY(cudaEventRecord(sl.back, c->s_out));
+                }
             }
-            H_TRY(cudaEventRecord(c->ev_round, c->s_out));
+            if (swap) H_TRY(cudaEventRecord(c->ev_round, c->s_out));
             // a6, the table half: fold by the challenge the last chunk's kernel drew (no gates in this launch)
             uint64_t *out = (j & 1) ? c->d_T1 : c->d_T0;
             const uint32_t half = 1u << (s - j - 1);

@@ -27,8 +27,9 @@ def vc():
     return v
 
 
-def _prove_hosted(vc, c, seed, chunk_log, layerwise=False):
+def _prove_hosted(vc, c, seed, chunk_log, layerwise=False, swap=False):
     gc = vc.Circuit(c, hosted_chunk_log=chunk_log)
+    gc.set_hosted_weights(swap)
     gc.set_input(c.input)
     gc.evaluate()
     ev_bytes = gc.hosted_bytes()
@@ -60,23 +61,27 @@ def test_hosted_circuit_transcript_is_the_oracles(vc, make, seed, chunk_logs):
     want_out, want_tr, want_z, want_claim = oc.prove(c.input, seed)
     V = oc.evaluate(c.input)
     for chunk_log in chunk_logs:
-        for layerwise in (False, True):
-            gc, out, tr, ev_bytes = _prove_hosted(vc, c, seed, chunk_log, layerwise)
+        for layerwise, swap in ((False, False), (True, False), (False, True), (True, True)):
+            gc, out, tr, ev_bytes = _prove_hosted(vc, c, seed, chunk_log, layerwise, swap)
             for i in range(c.d + 1):
                 assert np.array_equal(gc.values(i), V[i]), (c.name, chunk_log, i)
-            assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (c.name, chunk_log, layerwise)
+            assert np.array_equal(out, want_out) and np.array_equal(tr, want_tr), (c.name, chunk_log, layerwise, swap)
             z, claim, ctr = gc.state()
             assert claim == want_claim and np.array_equal(z[:c.log_input], want_z[:c.log_input])
             assert gc.verify(c.input, out, seed, tr) == (True, 0, 0)
-            # traffic: evaluation streams each record once; the proof streams, per message, 9 B of records per gate plus
-            # 8 B of weights each way (round 0 of a layer computes the weights instead of reading them)
+            # traffic: evaluation streams each record once; the proof streams, per message, 9 B of records per gate - and,
+            # when the weights are swapped through the host, 8 B of weights each way on top (round 0 of a layer computes
+            # them instead of reading them); recomputed weights never cross the link
             first = 1 if c.sum_output else 0
             gates = [1 << c.layers[i].log_size for i in range(first, c.d)]
             rounds = [2 * c.log_below(i) for i in range(first, c.d)]
             assert ev_bytes == (9 * sum(gates), 0)
             h2d, d2h = gc.hosted_bytes()
-            assert h2d == sum(n * (17 * r - 8) for n, r in zip(gates, rounds))
-            assert d2h == sum(n * 8 * r for n, r in zip(gates, rounds))
+            if swap:
+                assert h2d == sum(n * (17 * r - 8) for n, r in zip(gates, rounds))
+                assert d2h == sum(n * 8 * r for n, r in zip(gates, rounds))
+            else:
+                assert h2d == sum(n * 9 * r for n, r in zip(gates, rounds)) and d2h == 0
             gc.close()
 
 
@@ -84,7 +89,12 @@ def test_hosted_matches_golden_digest_at_config_2_size(vc):
     """BASELINE.json config 2 (F2, n = 2^20) with every message streamed in pieces of 2^17 gates: the oracle's golden digests."""
     c = W.config(2)
     seed = W.challenge_seed(2)
-    gc, out, tr, _ = _prove_hosted(vc, c, seed, 17)
+    for swap in (False, True):
+        _check_config2(vc, c, seed, swap)
+
+
+def _check_config2(vc, c, seed, swap):
+    gc, out, tr, _ = _prove_hosted(vc, c, seed, 17, swap=swap)
     g = {}
     with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config2.txt")) as f:
         for line in f:
@@ -117,6 +127,9 @@ def test_hosted_handle_rules(vc):
     assert e.value.code == 3
     with pytest.raises(vc.VCError) as e:
         gr.hosted_bytes()
+    assert e.value.code == 3
+    with pytest.raises(vc.VCError) as e:
+        gr.set_hosted_weights(True)
     assert e.value.code == 3
     gr.close()
     for bad in (7, 29):
