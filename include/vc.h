@@ -62,7 +62,9 @@ int vc_circuit_load(const vc_layer *layers, uint32_t d, uint32_t log_input, vc_c
  * copies of neighbouring pieces overlapping the kernel on internal streams.  The weights are either recomputed from the
  * record for every message (default: nothing but 9 B per gate and message crosses the host link) or swapped through the
  * host array as the paper words it (vc_hosted_set_weights(c, 1): + 8 B per gate up and 8 B down per message, the pending
- * update of the previous challenge applied when the piece comes back).  vc_evaluate streams the records once per
+ * update of the previous challenge applied when the piece comes back).  A layer of at most 2^chunk_log gates is copied
+ * ONCE and stays in its slot, weights included, for all of its messages (the paper's copy-once-per-layer approach,
+ * PAPER.md:157 §5.1.2): only wider layers are streamed per message.  vc_evaluate streams the records once per
  * layer.  Every other call (vc_prove_layer, vc_prove, vc_run_host, vc_verify_transcript, sizes) behaves as for a resident
  * circuit and produces the same words; vc_set_schedule accepts only 2 for such a handle (and 2 only for such a handle),
  * vc_verify_transcript_device returns VC_ERR_STATE (its wiring sums need device-resident records). */

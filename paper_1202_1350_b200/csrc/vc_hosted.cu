@@ -22,6 +22,8 @@
 //       array; a piece brings its weights along (8 B per gate up), the kernel applies the pending update of the previous
 //       challenge (it exists only once every piece of the previous message has been reduced) before the gate's
 //       contribution, and the updated weights travel back on the copy-out stream (8 B per gate down): 25 B per gate and message.
+// A layer that fits ONE slot is copied once and stays there for all of its messages, weights included: the paper's
+// "copy-once-per-layer approach" (§5.1.2); only wider layers are streamed per message.
 // Round 0 of a layer computes beta either way (a3) and, for layer 0, the start claim.  The message of a round is the sum over
 // pieces of the per-piece sums (a device accumulator; the kernel of the last piece writes the message and draws the
 // challenge).  Fold tables, line restriction and the sum gate are the resident kernels of the streaming schedule.  Results
@@ -239,25 +241,31 @@ int hosted_prove_layer(vc_circuit *c, uint32_t layer, uint64_t seed, uint64_t *d
     if (rc != VC_OK) return rc;
     uint64_t *tr = d_tr;
     uint32_t k = 0;
+    // A layer that fits one slot is copied ONCE and stays there, weights included, for all of its messages: the paper's
+    // "copy-once-per-layer approach" (§5.1.2, the one its experiments used); only wider layers pay per message.
+    const bool once = nchunks == 1;
     for (int phase = 1; phase <= 2; phase++) {
         const uint64_t *tab = Vb;
         for (uint32_t j = 0; j < s; j++) {
             const int mode = (phase == 1 && j == 0) ? 0 : ((phase == 2 && j == 0) ? 2 : 1);
-            const bool swap = c->hosted_swap;
+            const bool swap = c->hosted_swap && !once;
             if (swap && mode != 0) H_TRY(cudaStreamWaitEvent(c->s_in, c->ev_round, 0));  // the weights of the previous message are back on the host
             for (uint32_t q = 0; q < nchunks; q++, k++) {
                 const uint32_t g0 = q * ch, cnt = std::min(ch, n - g0);
-                auto &sl = c->slot[k & 1];
-                if ((rc = chunk_in(c, layer, k, g0, cnt, swap && mode != 0)) != VC_OK) return rc;
-                H_TRY(cudaStreamWaitEvent(st, sl.ready, 0));
+                auto &sl = c->slot[once ? 0 : (k & 1)];
+                if (!once || mode == 0) {
+                    if ((rc = chunk_in(c, layer, once ? 0 : k, g0, cnt, swap && mode != 0)) != VC_OK) return rc;
+                    H_TRY(cudaStreamWaitEvent(st, sl.ready, 0));
+                }
                 const int last = q + 1 == nchunks, set_claim = layer == 0 && mode == 0;
+                const int recompute = (swap || once) ? 0 : 1;        // once: the weights stay in the slot between messages
                 const uint32_t gg = grid_for(cnt, c->sm_count);
                 if (phase == 1)
                     VC_LAUNCH(VC_K_ROUND, k_cem_round<1>, gg, RED_BLOCK, 0, st, sl.type, sl.in1, sl.in2, sl.P, g0, cnt, si, c->d_V[layer], tab, Vb, S, j, s,
-                              mode, last, set_claim, swap ? 0 : 1, c->d_part, c->d_acc, tr);
+                              mode, last, set_claim, recompute, c->d_part, c->d_acc, tr);
                 else
                     VC_LAUNCH(VC_K_ROUND, k_cem_round<2>, gg, RED_BLOCK, 0, st, sl.type, sl.in1, sl.in2, sl.P, g0, cnt, si, c->d_V[layer], tab, Vb, S, j, s,
-                              mode, last, set_claim, swap ? 0 : 1, c->d_part, c->d_acc, tr);
+                              mode, last, set_claim, recompute, c->d_part, c->d_acc, tr);
                 H_TRY(cudaEventRecord(sl.done, st));
                 if (swap) {                                                              // swap the piece back
                     H_TRY(cudaStreamWaitEvent(c->s_out, sl.done, 0));
