@@ -62,16 +62,19 @@ def algorithmic_counts(c):
                 modmul=sum(l["modmul"] + l["modmul_eval"] for l in per_layer))
 
 
+FUSED_SOURCES = ("fp61.cuh", "vc_state.cuh", "vc_kernels.cuh", "vc_fused.cu", "vc_fused.cuh", "vc_fused_line.cuh", "vc_fused_small.cuh",
+                 "vc_fused_thin.cuh", "vc_fused_wide.cuh", "vc_cluster.cuh")
+
+
 def csrc_digest() -> str:
-    """SHA-256 over the kernel sources (csrc/*, include/vc.h, sorted by name): ties profiles/r02_traffic.json to a build."""
+    """SHA-256 over the device sources the fused proof kernels (k_fused<*>, k_cluster, k_eval_all) are compiled from — the
+    translation unit vc_fused.cu and every .cuh it includes: ties profiles/r02_traffic.json to the kernel it was captured on."""
     import hashlib
     h = hashlib.sha256()
     base = os.path.join(ROOT, "paper_1202_1350_b200", "csrc")
-    for name in sorted(os.listdir(base)):
+    for name in FUSED_SOURCES:
         with open(os.path.join(base, name), "rb") as f:
             h.update(name.encode()); h.update(f.read())
-    with open(os.path.join(ROOT, "include", "vc.h"), "rb") as f:
-        h.update(b"vc.h"); h.update(f.read())
     return h.hexdigest()
 
 
@@ -427,9 +430,9 @@ def run_ours(args):
             if k == 2 and args.schedule == 0 and tj.get("kernel_kind") == dom:
                 if tj.get("csrc_sha256") == csrc_digest():    # the capture is of THIS kernel source: else no traffic figure
                     traffic = int(tj["dram_bytes_read"]) + int(tj["dram_bytes_write"])
-                    traffic_src = f"profiles/r02_traffic.json (ncu --set full capture of commit {tj.get('commit', '?')}, same csrc/ + vc.h digest as this build, one launch)"
+                    traffic_src = f"profiles/r02_traffic.json (ncu --set full capture of commit {tj.get('commit', '?')}, same digest of the fused kernels' sources as this build, one launch)"
                 else:
-                    traffic_src = "profiles/r02_traffic.json is of another kernel source (csrc digest differs): no traffic figure for this build"
+                    traffic_src = "profiles/r02_traffic.json is of another kernel source (digest of the fused kernels' sources differs): no traffic figure for this build"
         except Exception:
             pass
         roofline = {"bound": "hbm" if dom_hbm_ms >= dom_alu_ms else "alu", "kernel": dom,
